@@ -1,0 +1,133 @@
+/*
+ * ocfd.h -- C ABI of the B200-native RHS / RK3 hot path of the OpenCFD-SCU finite-difference DNS method
+ * (arxiv 2209.15333; citations "PAPER.md:Lnnn" are lines of /root/reference/PAPER.md, "DESIGN R-n" are the
+ * readings registered in DESIGN.md section 3).
+ *
+ * One structured block on ONE GPU (sm_100a), fp64 throughout.  All field pointers are DEVICE
+ * pointers unless a name says "host".  The library allocates no field memory: the caller (PyTorch in the Python
+ * binding) owns U, dU, the metric fields, the boundary data and one scratch workspace.  Every call except
+ * ocfd_max_wavespeed and ocfd_rk3_steps_host only enqueues work on the stream given at init and returns.
+ *
+ * Layout: a field is a padded box [nz+8][ny+8][nx+8], x contiguous, 4 ghost layers per
+ * face (LAP = 4, the reach of the 7th-order stencils).  U and dU are component-major [5][nz+8][ny+8][nx+8] with
+ * components (rho, rho u, rho v, rho w, E) (eq. 5).  Interior index (i,j,k) lives at padded
+ * (i+4, j+4, k+4).  Edge and corner ghosts are never read nor written by any entry point.
+ *
+ * Errors: every entry point returns an ocfd_status; argument errors are detected synchronously and leave all
+ * buffers untouched; CUDA launch errors map to OCFD_ECUDA.  No global state; several contexts may coexist.
+ * There is no CPU fallback of any kind.
+ */
+#ifndef OCFD_H
+#define OCFD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ocfd_ctx ocfd_ctx; /* opaque; owns no device memory */
+
+typedef enum {
+    OCFD_OK = 0,
+    OCFD_EINVAL = -1,       /* bad argument (null pointer, bad size, inconsistent boundary pairing ...) */
+    OCFD_EWORKSPACE = -2,   /* workspace missing, misaligned or smaller than ocfd_workspace_bytes() */
+    OCFD_ECUDA = -3,        /* a CUDA runtime call or kernel launch failed */
+    OCFD_EUNSUPPORTED = -4, /* valid request this build does not implement */
+    OCFD_ESTATE = -5        /* call order violated (e.g. destroyed context) */
+} ocfd_status;
+
+typedef enum { OCFD_GRID_UNIFORM = 0, OCFD_GRID_STRETCHED = 1, OCFD_GRID_CURVILINEAR = 2 } ocfd_grid_kind;
+
+/* Inviscid reconstruction (Table 2 rows 6, 4, 2 and the hybrid of eq. 42). */
+typedef enum { OCFD_UD7 = 0, OCFD_WENO7 = 1, OCFD_WENO5 = 2, OCFD_HYBRID = 3 } ocfd_scheme;
+
+/* Boundary treatment of one face (DESIGN R-16; the paper prints no formulas). */
+typedef enum {
+    OCFD_BC_PERIODIC = 0,
+    OCFD_BC_WALL_ISOTHERMAL = 1,
+    OCFD_BC_SUPERSONIC_INFLOW = 2,
+    OCFD_BC_EXTRAP_OUTFLOW = 3
+} ocfd_bc;
+
+typedef struct {
+    int nx, ny, nz;   /* interior dimensions, each >= 8 */
+    int ng;           /* ghost layers; must be 4 */
+    ocfd_grid_kind grid_kind;
+    /* Metric data (eq. 3-4), device pointers, caller-owned, must outlive the context.
+     *   CURVILINEAR: metric[0..8] = xi_x xi_y xi_z eta_x eta_y eta_z zeta_x zeta_y zeta_z, metric[9] = J,
+     *                each a padded field including ghost values; consecutive k-planes are
+     *                metric_plane_stride doubles apart: (nx+8)*(ny+8) for full 3-D fields, 0 for a 2-D map
+     *                extruded in z (one padded plane per metric, the shape of the paper's ramp and
+     *                flat-plate grids).
+     *   STRETCHED:   metric[0], metric[4], metric[8] = padded 1-D arrays xi_x(i), eta_y(j), zeta_z(k) of
+     *                nx+8, ny+8, nz+8 doubles; the rest NULL.  J = (xi_x * eta_y) * zeta_z.
+     *   UNIFORM:     all NULL; spacing dx, dy, dz below.  xi_x = 1/dx ..., J = ((1/dx)(1/dy))(1/dz). */
+    const double *metric[10];
+    long long metric_plane_stride;
+    double dx, dy, dz;
+    /* Gas / flow parameters: ratio of specific heats, reference Mach, Reynolds and Prandtl
+     * numbers, reference temperature [K] and Sutherland constant [K] (DESIGN R-8: 110.4). */
+    double gamma, Ma, Re, Pr, T_ref, T_suth;
+    int inviscid;            /* 1: skip the viscous terms (rows a6, a7) */
+    ocfd_scheme scheme;
+    double theta1, theta2;   /* hybrid thresholds (0.02, 0.1); theta2 = +inf gives two levels */
+    double weno_eps;         /* epsilon of the WENO weights, applied to the J^-1-scaled split flux (DESIGN R-10) */
+    double sw_eps;           /* 0: eigenvalue split exactly as eq. 29; > 0: (lambda +- sqrt(lambda^2+eps^2))/2 */
+    ocfd_bc bc[6];           /* x-, x+, y-, y+, z-, z+; PERIODIC must be set on both faces of an axis */
+    double T_wall[6];        /* non-dimensional wall temperature of WALL faces */
+    /* Optional prescribed wall-normal velocity (blowing / suction) of WALL faces: padded 2-D device array over
+     * the two tangential axes, [slow+8][fast+8] with fast = x (or y on x-faces), else NULL. */
+    const double *wall_vn[6];
+    /* INFLOW faces: 5 padded 2-D device arrays of conserved variables, component-major [5][slow+8][fast+8]. */
+    const double *inflow[6];
+    void *workspace;         /* device scratch, 256-byte aligned, at least ocfd_workspace_bytes() */
+    size_t workspace_bytes;
+    void *stream;            /* cudaStream_t to enqueue on (0 = default stream) */
+} ocfd_params;
+
+/* Bytes of device scratch a context with these parameters needs; 0 if the parameters are invalid.  Pure. */
+size_t ocfd_workspace_bytes(const ocfd_params *p);
+
+/* Validate, copy the parameters, carve the workspace.  No field memory is allocated. */
+ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p);
+ocfd_status ocfd_destroy(ocfd_ctx *ctx);
+
+/* Row a1.  Set Dirichlet nodes (wall, inflow) then fill the 4 ghost layers of every face of U, in place,
+ * faces in the order x-, x+, y-, y+, z-, z+ (DESIGN R-16). */
+ocfd_status ocfd_fill_ghosts(ocfd_ctx *ctx, double *U);
+
+/* Rows a2-a7.  dU <- L(U) = -J sum_d d(F_d)/d(d) + J sum_d d(Fv_d)/d(d) (eq. 1) on interior points.
+ * Ghosts of U must be valid; ghosts of dU are left untouched; U is not modified (pure function of U). */
+ocfd_status ocfd_rhs(ocfd_ctx *ctx, const double *U, double *dU);
+
+/* Rows a1-a8.  One TVD-RK3 step (eq. 45): 3 x (fill ghosts, RHS, stage update), then a
+ * final ghost fill, in place on U. */
+ocfd_status ocfd_rk3_step(ocfd_ctx *ctx, double *U, double dt);
+
+/* The same nsteps steps end to end from HOST memory: copy U_host (5 padded fields, pinned or pageable) into the
+ * device buffer U_dev, step, copy back, synchronise the stream. */
+ocfd_status ocfd_rk3_steps_host(ocfd_ctx *ctx, double *U_host, double *U_dev, double dt, int nsteps);
+
+/* Row a9.  Lambda = max over interior points of sum_d (|d_x u + d_y v + d_z w| + c |grad d|) (DESIGN R-17);
+ * the caller sets dt = CFL / Lambda.  Writes one double to host_out and synchronises the stream. */
+ocfd_status ocfd_max_wavespeed(ocfd_ctx *ctx, const double *U, double *host_out);
+
+/* Hybrid-scheme parity report: theta (padded field, interior + the first ghost layer of each face written) and
+ * the per-interface scheme flags (0 UD7, 1 WENO7, 2 WENO5): flag_xyz is [3][nz+8][ny+8][nx+8] bytes and
+ * flag_xyz[d][point s] is the scheme of interface s+1/2 along direction d, s = -1 .. n-1.  Either output
+ * may be NULL.  Device pointers. */
+ocfd_status ocfd_debug_sensor(ocfd_ctx *ctx, const double *U, double *theta, unsigned char *flag_xyz);
+
+/* sizeof(ocfd_params) as compiled, so that a foreign-language mirror of the struct can check itself. */
+size_t ocfd_sizeof_params(void);
+
+/* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
+long long ocfd_launch_count(const ocfd_ctx *ctx);
+
+const char *ocfd_strerror(ocfd_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OCFD_H */

@@ -1,0 +1,209 @@
+// C ABI of libocfd_b200 (include/ocfd.h): argument validation, workspace carve-up, step orchestration.
+#include <math.h>
+#include <new>
+#include <string.h>
+
+#include "ocfd_internal.cuh"
+
+namespace {
+
+const uint64_t kMagic = 0x4f43464442323030ull;  // "OCFDB200"
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool valid_params(const ocfd_params *p) {
+    if (!p) return false;
+    if (p->ng != OCFD_NG) return false;
+    if (p->nx < 8 || p->ny < 8 || p->nz < 8) return false;
+    if ((long long)(p->nx + 8) * (p->ny + 8) * (p->nz + 8) > (1ll << 40)) return false;
+    if (!(p->gamma > 1.0) || !(p->Ma > 0.0) || !(p->weno_eps > 0.0) || !(p->sw_eps >= 0.0)) return false;
+    if (!p->inviscid && (!(p->Re > 0.0) || !(p->Pr > 0.0) || !(p->T_ref > 0.0) || !(p->T_suth >= 0.0))) return false;
+    if (p->scheme < OCFD_UD7 || p->scheme > OCFD_HYBRID) return false;
+    if (p->scheme == OCFD_HYBRID && (isnan(p->theta1) || isnan(p->theta2))) return false;
+    switch (p->grid_kind) {
+        case OCFD_GRID_UNIFORM:
+            if (!(p->dx > 0.0) || !(p->dy > 0.0) || !(p->dz > 0.0)) return false;
+            break;
+        case OCFD_GRID_STRETCHED:
+            if (!p->metric[0] || !p->metric[4] || !p->metric[8]) return false;
+            break;
+        case OCFD_GRID_CURVILINEAR:
+            for (int q = 0; q < 10; ++q)
+                if (!p->metric[q]) return false;
+            if (p->metric_plane_stride != 0 && p->metric_plane_stride != (long long)(p->nx + 8) * (p->ny + 8)) return false;
+            break;
+        default: return false;
+    }
+    for (int f = 0; f < 6; ++f) {
+        if (p->bc[f] < OCFD_BC_PERIODIC || p->bc[f] > OCFD_BC_EXTRAP_OUTFLOW) return false;
+        if (p->bc[f] == OCFD_BC_SUPERSONIC_INFLOW && !p->inflow[f]) return false;
+        if (p->bc[f] == OCFD_BC_WALL_ISOTHERMAL && !(p->T_wall[f] > 0.0)) return false;
+    }
+    for (int d = 0; d < 3; ++d)
+        if ((p->bc[2 * d] == OCFD_BC_PERIODIC) != (p->bc[2 * d + 1] == OCFD_BC_PERIODIC)) return false;
+    return true;
+}
+
+struct Carve { size_t prim, theta, Fv, Un, dUw, scal, total; };
+
+Carve carve(const ocfd_params *p) {
+    const size_t np = (size_t)(p->nx + 8) * (p->ny + 8) * (p->nz + 8);
+    const size_t fb = align_up(np * sizeof(double), 256);
+    Carve c;
+    size_t off = 0;
+    c.prim = off; off += align_up(P_NF * np * sizeof(double), 256);
+    c.theta = off; off += fb;
+    c.Fv = off; off += p->inviscid ? 0 : align_up(12 * np * sizeof(double), 256);
+    c.Un = off; off += align_up(5 * np * sizeof(double), 256);
+    c.dUw = off; off += align_up(5 * np * sizeof(double), 256);
+    c.scal = off; off += 256;
+    c.total = off;
+    return c;
+}
+
+bool live(const ocfd_ctx *c) { return c && c->magic == kMagic; }
+
+}  // namespace
+
+extern "C" {
+
+size_t ocfd_workspace_bytes(const ocfd_params *p) {
+    if (!valid_params(p)) return 0;
+    return carve(p).total;
+}
+
+ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
+    if (!out) return OCFD_EINVAL;
+    *out = nullptr;
+    if (!valid_params(p)) return OCFD_EINVAL;
+    const Carve cv = carve(p);
+    if (!p->workspace || ((uintptr_t)p->workspace & 255) || p->workspace_bytes < cv.total) return OCFD_EWORKSPACE;
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return OCFD_ECUDA;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return OCFD_ECUDA;
+    if (major < 10) return OCFD_EUNSUPPORTED;  // sm_100a only; there is no other code path
+    ocfd_ctx *c = new (std::nothrow) ocfd_ctx();
+    if (!c) return OCFD_EINVAL;
+    c->magic = kMagic;
+    c->p = *p;
+    c->stream = (cudaStream_t)p->stream;
+    GridDesc &g = c->g;
+    g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
+    g.nxp = p->nx + 8; g.nyp = p->ny + 8; g.nzp = p->nz + 8;
+    g.sy = g.nxp; g.sz = (long long)g.nxp * g.nyp; g.np = g.sz * g.nzp;
+    g.kind = p->grid_kind;
+    for (int q = 0; q < 10; ++q) g.met[q] = p->metric[q];
+    g.msk = p->metric_plane_stride;
+    g.ux = g.uy = g.uz = g.uJ = 0.0;
+    if (p->grid_kind == OCFD_GRID_UNIFORM) {
+        g.ux = 1.0 / p->dx; g.uy = 1.0 / p->dy; g.uz = 1.0 / p->dz;
+        g.uJ = (g.ux * g.uy) * g.uz;
+    }
+    for (int d = 0; d < 3; ++d) g.periodic[d] = p->bc[2 * d] == OCFD_BC_PERIODIC;
+    GasDesc &s = c->gas;
+    s.gamma = p->gamma; s.gm1 = p->gamma - 1.0; s.Ma = p->Ma; s.gM2 = p->gamma * p->Ma * p->Ma; s.invMa = 1.0 / p->Ma;
+    s.inv2g = 1.0 / (2.0 * p->gamma);
+    s.w0 = (3.0 - p->gamma) / (2.0 * (p->gamma - 1.0));
+    s.tgm1 = 2.0 * (p->gamma - 1.0);
+    s.suth = p->inviscid ? 0.0 : p->T_suth / p->T_ref;
+    s.invRe = p->inviscid ? 0.0 : 1.0 / p->Re;
+    s.kfac = p->inviscid ? 0.0 : 1.0 / ((p->gamma - 1.0) * p->Ma * p->Ma * p->Pr * p->Re);
+    s.weno_eps = p->weno_eps; s.sw_eps = p->sw_eps; s.theta1 = p->theta1; s.theta2 = p->theta2;
+    char *w = (char *)p->workspace;
+    c->prim = (double *)(w + cv.prim);
+    c->theta = (double *)(w + cv.theta);
+    c->Fv = (double *)(w + cv.Fv);
+    c->Un = (double *)(w + cv.Un);
+    c->dUw = (double *)(w + cv.dUw);
+    c->scal = (double *)(w + cv.scal);
+    c->flags = nullptr;
+    c->launches = 0;
+    *out = c;
+    return OCFD_OK;
+}
+
+ocfd_status ocfd_destroy(ocfd_ctx *c) {
+    if (!live(c)) return OCFD_ESTATE;
+    c->magic = 0;
+    delete c;
+    return OCFD_OK;
+}
+
+ocfd_status ocfd_fill_ghosts(ocfd_ctx *c, double *U) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U) return OCFD_EINVAL;
+    return launch_fill_ghosts(c, U);
+}
+
+ocfd_status ocfd_rhs(ocfd_ctx *c, const double *U, double *dU) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U || !dU || U == dU) return OCFD_EINVAL;
+    ocfd_status st;
+    if ((st = launch_prim(c, U)) != OCFD_OK) return st;
+    if (c->p.scheme == OCFD_HYBRID && (st = launch_sensor(c, U)) != OCFD_OK) return st;
+    if ((st = launch_inviscid(c, U, dU)) != OCFD_OK) return st;
+    if (!c->p.inviscid && (st = launch_viscous(c, U, dU)) != OCFD_OK) return st;
+    return OCFD_OK;
+}
+
+ocfd_status ocfd_rk3_step(ocfd_ctx *c, double *U, double dt) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U || !(dt == dt)) return OCFD_EINVAL;
+    ocfd_status st;
+    for (int s = 0; s < 3; ++s) {
+        if ((st = launch_fill_ghosts(c, U)) != OCFD_OK) return st;
+        if ((st = ocfd_rhs(c, U, c->dUw)) != OCFD_OK) return st;
+        if ((st = launch_rk_update(c, c->Un, U, c->dUw, dt, s)) != OCFD_OK) return st;
+    }
+    return launch_fill_ghosts(c, U);
+}
+
+ocfd_status ocfd_rk3_steps_host(ocfd_ctx *c, double *U_host, double *U_dev, double dt, int nsteps) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U_host || !U_dev || nsteps < 0) return OCFD_EINVAL;
+    const size_t bytes = (size_t)5 * c->g.np * sizeof(double);
+    if (cudaMemcpyAsync(U_dev, U_host, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) return OCFD_ECUDA;
+    for (int n = 0; n < nsteps; ++n) {
+        ocfd_status st = ocfd_rk3_step(c, U_dev, dt);
+        if (st != OCFD_OK) return st;
+    }
+    if (cudaMemcpyAsync(U_host, U_dev, bytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return OCFD_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return OCFD_ECUDA;
+    return OCFD_OK;
+}
+
+ocfd_status ocfd_max_wavespeed(ocfd_ctx *c, const double *U, double *host_out) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U || !host_out) return OCFD_EINVAL;
+    return launch_wavespeed(c, U, host_out);
+}
+
+ocfd_status ocfd_debug_sensor(ocfd_ctx *c, const double *U, double *theta, unsigned char *flag_xyz) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U) return OCFD_EINVAL;
+    ocfd_status st;
+    if ((st = launch_prim(c, U)) != OCFD_OK) return st;
+    if ((st = launch_sensor(c, U)) != OCFD_OK) return st;
+    if (theta && cudaMemcpyAsync(theta, c->theta, c->g.np * sizeof(double), cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+        return OCFD_ECUDA;
+    if (flag_xyz && (st = launch_flags(c, flag_xyz)) != OCFD_OK) return st;
+    return OCFD_OK;
+}
+
+size_t ocfd_sizeof_params(void) { return sizeof(ocfd_params); }
+
+long long ocfd_launch_count(const ocfd_ctx *c) { return live(c) ? c->launches : -1; }
+
+const char *ocfd_strerror(ocfd_status s) {
+    switch (s) {
+        case OCFD_OK: return "ok";
+        case OCFD_EINVAL: return "invalid argument";
+        case OCFD_EWORKSPACE: return "workspace missing, misaligned or too small";
+        case OCFD_ECUDA: return "CUDA runtime or launch error";
+        case OCFD_EUNSUPPORTED: return "unsupported (this library runs on sm_100a only)";
+        case OCFD_ESTATE: return "invalid or destroyed context";
+    }
+    return "unknown status";
+}
+
+}  // extern "C"

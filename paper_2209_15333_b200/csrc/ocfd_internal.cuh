@@ -1,0 +1,102 @@
+// Internal declarations shared by the CUDA translation units of libocfd_b200 (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "ocfd.h"
+
+#define OCFD_NG 4
+
+// Grid description handed to kernels by value.
+struct GridDesc {
+    int nx, ny, nz;        // interior
+    int nxp, nyp, nzp;     // padded
+    long long sy, sz, np;  // strides in doubles (x stride is 1), padded points per field
+    int kind;              // ocfd_grid_kind
+    const double *met[10];
+    long long msk;         // metric k-plane stride (curvilinear)
+    double ux, uy, uz;     // uniform: 1/dx, 1/dy, 1/dz
+    double uJ;             // uniform: J
+    int periodic[3];
+};
+
+// Gas / scheme constants handed to kernels by value.
+struct GasDesc {
+    double gamma, gm1, Ma, gM2, invMa;  // gM2 = gamma Ma^2
+    double inv2g;                       // 1/(2 gamma)
+    double w0;                          // (3-gamma)/(2(gamma-1))   (eq. 26)
+    double tgm1;                        // 2(gamma-1)
+    double suth;                        // T_suth/T_ref
+    double invRe, kfac;                 // 1/Re, 1/((gamma-1) Ma^2 Pr Re)
+    double weno_eps, sw_eps, theta1, theta2;
+};
+
+struct ocfd_ctx {
+    uint64_t magic;
+    ocfd_params p;
+    GridDesc g;
+    GasDesc gas;
+    cudaStream_t stream;
+    // workspace carve-up (device pointers)
+    double *prim;    // [6][np]: u v w T c p
+    double *theta;   // [np]
+    double *Fv;      // [12][np]
+    double *Un;      // [5][np]
+    double *dUw;     // [5][np]
+    double *scal;    // small scalar area (wavespeed result)
+    unsigned char *flags;  // [3][np] bytes (debug only)
+    long long launches;
+};
+
+// prim field order
+enum { P_U = 0, P_V = 1, P_W = 2, P_T = 3, P_C = 4, P_P = 5, P_NF = 6 };
+
+// ---------------------------------------------------------------- metric access
+// padded linear index of (ip,jp,kp)
+__device__ __forceinline__ long long pidx(const GridDesc &g, int ip, int jp, int kp) {
+    return (long long)kp * g.sz + (long long)jp * g.sy + ip;
+}
+
+template <int KIND>
+struct Met {
+    // metric row of direction d at padded point (ip,jp,kp): (d_x, d_y, d_z)
+    __device__ __forceinline__ static void row(const GridDesc &g, int d, int ip, int jp, int kp, double &a, double &b,
+                                               double &c) {
+        if (KIND == OCFD_GRID_UNIFORM) {
+            a = d == 0 ? g.ux : 0.0;
+            b = d == 1 ? g.uy : 0.0;
+            c = d == 2 ? g.uz : 0.0;
+        } else if (KIND == OCFD_GRID_STRETCHED) {
+            a = d == 0 ? __ldg(g.met[0] + ip) : 0.0;
+            b = d == 1 ? __ldg(g.met[4] + jp) : 0.0;
+            c = d == 2 ? __ldg(g.met[8] + kp) : 0.0;
+        } else {
+            long long mi = (long long)kp * g.msk + (long long)jp * g.sy + ip;
+            a = __ldg(g.met[3 * d] + mi);
+            b = __ldg(g.met[3 * d + 1] + mi);
+            c = __ldg(g.met[3 * d + 2] + mi);
+        }
+    }
+    __device__ __forceinline__ static double J(const GridDesc &g, int ip, int jp, int kp) {
+        if (KIND == OCFD_GRID_UNIFORM) return g.uJ;
+        if (KIND == OCFD_GRID_STRETCHED) return (__ldg(g.met[0] + ip) * __ldg(g.met[4] + jp)) * __ldg(g.met[8] + kp);
+        return __ldg(g.met[9] + (long long)kp * g.msk + (long long)jp * g.sy + ip);
+    }
+};
+
+// ---------------------------------------------------------------- kernel launchers (host side)
+ocfd_status launch_fill_ghosts(ocfd_ctx *c, double *U);
+ocfd_status launch_prim(ocfd_ctx *c, const double *U);
+ocfd_status launch_sensor(ocfd_ctx *c, const double *U);
+ocfd_status launch_flags(ocfd_ctx *c, unsigned char *flags);
+ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU);
+ocfd_status launch_viscous(ocfd_ctx *c, const double *U, double *dU);
+ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage);
+ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
+
+#define OCFD_CHECK_LAUNCH(ctx)                                  \
+    do {                                                        \
+        (ctx)->launches++;                                      \
+        if (cudaGetLastError() != cudaSuccess) return OCFD_ECUDA; \
+    } while (0)

@@ -283,7 +283,7 @@ def flat_plate(nx=1024, ny=128, nz=128, seed=20224, scheme="weno7", nsteps=50, L
 
 # --------------------------------------------------------------------------- config 5: ramp
 def ramp(nx=2048, ny=300, nz=256, seed=20225, scheme="hybrid", theta2=np.inf, nsteps=20, dz=0.1,
-         x0=-120.0, x1=84.8, H=30.0, dy1=0.004, nmodes=64, rms=0.05):
+         x0=-120.0, x1=84.8, H=60.0, dy1=0.004, nmodes=64, rms=0.05):
     """Mach 2.9, 24-degree compression-ramp-shaped curvilinear grid, z-extruded 2-D map (config 5).
 
     Wall y_w(x) = tan24 (x + sqrt(x^2 + d^2))/2 - tan24 d/2 (smoothed corner, d = 2), x uniform,

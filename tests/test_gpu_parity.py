@@ -1,0 +1,225 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on seeded inputs.
+
+Tolerances (BASELINE.json north_star): relative L-inf <= 1e-11 per RHS, <= 1e-9 after 100 RK3 steps on smooth
+cases; hybrid-scheme flags exact except within 1e-12 of a threshold (counted and reported).
+Error metric: per conserved component m, max_i |gpu - ora| / max_i |ora| over interior points;
+when max|ora_m| is (numerically) zero the error is taken relative to max|U_m|.
+"""
+import numpy as np
+import pytest
+
+from paper_2209_15333_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+NG = 4
+INT = (slice(None), slice(NG, -NG), slice(NG, -NG), slice(NG, -NG))
+TOL_RHS = 1e-11
+TOL_100 = 1e-9
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2209_15333_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def Oracle():
+    from oracle.oracle import Oracle
+    return Oracle
+
+
+def rel_linf(gpu, ora, U, floor=0.0):
+    """max|gpu-ora| / max|ora| per component.  `floor` guards components whose exact value is zero or small by
+    cancellation (v and w momentum of a 2-D boundary layer, a steady profile): there the round-off of either side
+    scales with the terms that cancel, not with their sum, so the denominator is never taken below `floor`
+    (callers pass 1e-3 * Lambda_max * max|U|, Lambda = the wavespeed sum of DESIGN section 2, i.e. 0.1 % of the
+    size of dU/dt's individual terms)."""
+    errs = []
+    for m in range(5):
+        den = max(np.abs(ora[m]).max(), floor)
+        if den < 1e-300:
+            den = np.abs(U[m]).max()
+        errs.append(np.abs(gpu[m] - ora[m]).max() / den)
+    return np.array(errs)
+
+
+def term_floor(Oracle, case, U_full):
+    return 1e-3 * Oracle(case).max_wavespeed(U_full) * np.abs(U_full[INT]).max()
+
+
+def run_rhs_both(B, Oracle, case, fill=True):
+    o = Oracle(case)
+    U = case.U0.copy()
+    if fill:
+        o.fill_ghosts(U)
+    ref = o.rhs(U)
+    s = B.Solver(case)
+    Ud = s.to_device(U)
+    dUd = s.rhs(Ud)
+    s.torch.cuda.synchronize()
+    got = dUd.cpu().numpy()
+    assert np.array_equal(Ud.cpu().numpy(), U), "ocfd_rhs must not modify U"
+    ghost = np.ones(got.shape, dtype=bool)
+    ghost[INT] = False
+    assert np.all(got[ghost] == 0.0), "ocfd_rhs must leave the ghosts of dU untouched"
+    s.close()
+    return got[INT], ref[INT], U[INT]
+
+
+# sizes span several tiles of every kernel (x tile 56, y/z tile 20, viscous blocks 32x4x2) with ragged tails
+@pytest.mark.parametrize("scheme", ["ud7", "weno7", "weno5", "hybrid"])
+@pytest.mark.parametrize("grid", ["uniform", "stretched", "wavy"])
+def test_rhs_parity_smooth_periodic(B, Oracle, grid, scheme):
+    case = W.smooth_periodic(70, 45, 23, grid=grid, scheme=scheme, Re=150.0, seed=3)
+    got, ref, U = run_rhs_both(B, Oracle, case)
+    err = rel_linf(got, ref, U)
+    assert err.max() <= TOL_RHS, err
+
+
+@pytest.mark.parametrize("scheme", ["ud7", "weno7"])
+def test_rhs_parity_inviscid_only_and_sw_eps(B, Oracle, scheme):
+    case = W.smooth_periodic(58, 21, 41, grid="wavy", scheme=scheme, inviscid=True, seed=5)
+    case.sw_eps = 0.02
+    got, ref, U = run_rhs_both(B, Oracle, case)
+    assert rel_linf(got, ref, U).max() <= TOL_RHS
+
+
+def test_rhs_freestream_is_zero_to_roundoff(B, Oracle):
+    for grid in ("uniform", "stretched"):
+        case = W.smooth_periodic(60, 24, 22, grid=grid, scheme="weno7")
+        shp = case.padded_shape
+        one = np.ones(shp)
+        p = 1.1 * 0.9 / (case.gamma * case.Ma ** 2)
+        case.U0 = np.ascontiguousarray(W.cons_from_prim(1.1 * one, 0.8 * one, -0.3 * one, 0.45 * one, p * one, case.gamma))
+        got, ref, U = run_rhs_both(B, Oracle, case)
+        scale = np.abs(U).max() * max(np.abs(m).max() for m in case.metrics[:9])
+        assert np.abs(got).max() <= 1e-12 * scale
+        assert np.abs(got - ref).max() <= 1e-12 * scale
+
+
+def flag_report(B, Oracle, case, U):
+    """Compare sensor decisions; returns (mismatches outside the 1e-12 band, interfaces inside the band)."""
+    o = Oracle(case)
+    th_ref = o.sensor(U)
+    s = B.Solver(case)
+    th_gpu, fl_gpu = s.debug_sensor(s.to_device(U))
+    s.torch.cuda.synchronize()
+    th_gpu, fl_gpu = th_gpu.cpu().numpy(), fl_gpu.cpu().numpy()
+    s.close()
+    I = slice(NG, -NG)
+    assert np.abs(th_gpu[I, I, I] - th_ref[I, I, I]).max() <= 1e-13
+    bad = near = total = 0
+    hist = np.zeros(3, dtype=np.int64)
+    for d in range(3):
+        fl_ref = o.flags(th_ref, d)
+        sl = [I, I, I]
+        sl[2 - d] = slice(NG - 1, -NG)                     # interfaces s = -1 .. n-1 along d
+        sl = tuple(sl)
+        sh = [0, 0, 0]
+        sh[2 - d] = 1
+        a = th_ref[sl]
+        b = np.roll(th_ref, -1, axis=2 - d)[sl]
+        Th = np.maximum(a, b)
+        band = (np.abs(Th - case.theta1) <= 1e-12) | (np.abs(Th - case.theta2) <= 1e-12)
+        diff = fl_gpu[d][sl] != fl_ref[sl]
+        bad += int((diff & ~band).sum())
+        near += int(band.sum())
+        total += diff.size
+        hist += np.bincount(fl_ref[sl].ravel(), minlength=3)[:3]
+    return bad, near, total, hist
+
+
+def test_hybrid_sensor_decisions_and_rhs_on_shocked_field(B, Oracle):
+    case = W.shocked_periodic(44, theta1=0.02, theta2=0.1)
+    o = Oracle(case)
+    U = o.fill_ghosts(case.U0.copy())
+    bad, near, total, hist = flag_report(B, Oracle, case, U)
+    print(f"hybrid flags: {total} interfaces, {near} within 1e-12 of a threshold (excluded), {bad} mismatches; "
+          f"UD7/WENO7/WENO5 = {hist.tolist()}")
+    assert bad == 0
+    assert np.all(hist > 0)
+    got, ref, Ui = run_rhs_both(B, Oracle, case)
+    assert rel_linf(got, ref, Ui).max() <= TOL_RHS
+
+
+def test_fill_ghosts_matches_oracle_on_wall_inflow_outflow(B, Oracle):
+    for case in (W.flat_plate(nx=60, ny=26, nz=12), W.ramp(nx=48, ny=30, nz=10, nmodes=8)):
+        rng = np.random.default_rng(2)
+        U = np.ascontiguousarray(case.U0 * (1.0 + 0.02 * rng.uniform(-1, 1, case.U0.shape)))
+        ref = Oracle(case).fill_ghosts(U.copy())
+        s = B.Solver(case)
+        Ud = s.fill_ghosts(s.to_device(U))
+        s.torch.cuda.synchronize()
+        got = Ud.cpu().numpy()
+        s.close()
+        # every point the oracle wrote (and only those) must agree; copies are exact, wall arithmetic to round-off
+        assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max()
+        untouched = ref == U                     # edges, corners and the interior away from Dirichlet nodes
+        assert np.array_equal(got[untouched], U[untouched])
+
+
+@pytest.mark.parametrize("which", ["plate", "ramp", "ramp3level"])
+def test_rhs_parity_with_walls(B, Oracle, which):
+    if which == "plate":
+        case = W.flat_plate(nx=72, ny=44, nz=24)
+    else:
+        case = W.ramp(nx=64, ny=44, nz=24, nmodes=12, theta2=np.inf if which == "ramp" else 0.1)
+    got, ref, U = run_rhs_both(B, Oracle, case)
+    floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
+    err = rel_linf(got, ref, U, floor)
+    print(which, "rel Linf per component", err, "floor", floor, "max|ref|", np.abs(ref).max(axis=(1, 2, 3)))
+    assert err.max() <= TOL_RHS
+
+
+def step_both(B, Oracle, case, nsteps, check_every=None):
+    o = Oracle(case)
+    U = o.fill_ghosts(case.U0.copy())
+    dt = case.cfl / o.max_wavespeed(U)
+    s = B.Solver(case)
+    Ud = s.to_device(U)
+    lam = s.max_wavespeed(Ud)
+    assert lam == pytest.approx(case.cfl / dt, rel=1e-13)
+    worst = 0.0
+    for n in range(nsteps):
+        o.rk3_step(U, dt)
+        s.rk3_step(Ud, dt)
+        if check_every and ((n + 1) % check_every == 0 or n == nsteps - 1):
+            got = Ud.cpu().numpy()
+            worst = max(worst, rel_linf(got[INT], U[INT], U[INT], floor=1e-3 * np.abs(U[INT]).max()).max())
+    got = Ud.cpu().numpy()
+    s.close()
+    umax = np.abs(U[INT]).max()
+    err = rel_linf(got[INT], U[INT], U[INT], floor=1e-3 * umax)
+    # both sides leave the face ghosts filled; edges and corners are never touched by either
+    errg = max(np.abs(got[m] - U[m]).max() / max(np.abs(U[m]).max(), 1e-3 * umax) for m in range(5))
+    return max(worst, err.max(), errg), got, U
+
+
+def test_config1_tgv32_ten_steps(B, Oracle):
+    case = W.tgv(32)
+    err, _, _ = step_both(B, Oracle, case, case.nsteps, check_every=1)
+    print("config 1 (TGV 32^3, 10 steps): rel Linf", err)
+    assert err <= TOL_100
+
+
+def test_hundred_steps_smooth(B, Oracle):
+    case = W.tgv(24, nsteps=100)
+    err, _, _ = step_both(B, Oracle, case, 100, check_every=25)
+    print("TGV 24^3, 100 steps: rel Linf", err)
+    assert err <= TOL_100
+
+
+@pytest.mark.parametrize("which", ["plate", "ramp"])
+def test_twenty_steps_with_walls(B, Oracle, which):
+    case = W.flat_plate(nx=64, ny=40, nz=16) if which == "plate" else W.ramp(nx=64, ny=40, nz=16, nmodes=12)
+    err, got, ref = step_both(B, Oracle, case, 20)
+    print(which, "20 steps: rel Linf", err)
+    # hybrid decisions may legitimately flip where theta sits within round-off of a threshold; smooth twins stay tight
+    assert err <= (1e-9 if which == "plate" else 1e-7)
+    assert np.isfinite(got).all()
