@@ -1,0 +1,342 @@
+#!/usr/bin/env python
+"""bench.py -- grid-point RK3 steps per second of the ocfd hot path on B200 (one process per GPU).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
+
+A "step" is one TVD-RK3 step (3 x [ghost fill, primitives, sensor, inviscid x/y/z, viscous flux/div, RK update] + a
+final ghost fill) of the whole hot path on one synthetic workload.  The default workload is
+BASELINE.json's configs[4], the >=100M-point Mach 2.9 ramp grid that north_star's target names; it fits one GPU.
+N > 1 runs N independent replicas (north_star: no domain decomposition), value = sum over replicas.
+Prints ONE JSON line on rank 0 (contract: see the task statement; extra keys: roofline, cpu_baseline, kernels).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2209_15333_b200 import workloads as W  # noqa: E402
+
+METRIC = "grid_point_rk3_steps_per_sec"
+UNIT = "grid-point RK3 steps/s"
+
+# name -> (generator for the GPU workload, generator for the bounded CPU sample of the same workload, note)
+WORKLOADS = {
+    "ramp2048x300x256_hybrid": (lambda: W.ramp(), lambda: W.ramp(nx=512, ny=76, nz=32), "BASELINE configs[4]"),
+    "plate1024x128x128_weno7": (lambda: W.flat_plate(), lambda: W.flat_plate(nx=256, ny=64, nz=32), "BASELINE configs[3]"),
+    "hit256_hybrid": (lambda: W.hit(256, Mt=1.0, seed=20223, scheme="hybrid", nsteps=50),
+                      lambda: W.hit(64, Mt=1.0, seed=20223, scheme="hybrid", nsteps=50), "BASELINE configs[2]"),
+    "hit128_weno7": (lambda: W.hit(128), lambda: W.hit(64), "BASELINE configs[1]"),
+    "tgv32_weno7": (lambda: W.tgv(32), lambda: W.tgv(32), "BASELINE configs[0]"),
+    "ramp2048x300x256_weno7": (lambda: W.ramp(scheme="weno7"), lambda: W.ramp(nx=512, ny=76, nz=32, scheme="weno7"),
+                               "configs[4] grid with WENO7 everywhere (ALU-bound variant)"),
+    "ramp512x76x32_hybrid": (lambda: W.ramp(nx=512, ny=76, nz=32), lambda: W.ramp(nx=512, ny=76, nz=32), "small twin"),
+    "ramp1024x152x64_hybrid": (lambda: W.ramp(nx=1024, ny=152, nz=64), lambda: W.ramp(nx=512, ny=76, nz=32),
+                               "mid-size twin (ncu captures)"),
+    "ramp1024x152x64_weno7": (lambda: W.ramp(nx=1024, ny=152, nz=64, scheme="weno7"),
+                              lambda: W.ramp(nx=512, ny=76, nz=32, scheme="weno7"), "mid-size twin, WENO7 everywhere"),
+}
+DEFAULT_WORKLOAD = "ramp2048x300x256_hybrid"
+
+# Peaks: HBM from MEASURED_PEAKS.json (driver-written) else the profiling guide's fallback; fp64 from the committed
+# DFMA probe (profiles/fp64_peak_r01.md): 34.2 TFLOP/s sustained on this pool's B200 (nominal 148 SM x 64 lanes x 2 x
+# 1.965 GHz = 37.2).
+FP64_PEAK_TFLOPS = 34.2
+HBM_FALLBACK_GBS = 6650.0
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured"
+        except Exception:
+            pass
+    return HBM_FALLBACK_GBS, "fallback"
+
+
+# ----------------------------------------------------------------------------------------------------------
+# Algorithmic work per interior point and launch of each kernel class.  Bytes count every
+# field the kernel must read or write once; flops follow the operation counts of the formulas.
+def algorithmic(case, flag_hist=None):
+    hyb = case.scheme == "hybrid"
+    met3d = case.grid_kind == "curvilinear" and case.metrics[0].shape[0] > 1
+    P = float(np.prod(case.padded_shape)) / case.npoints            # padded / interior points
+    rec = {"ud7": 13.0, "weno7": 146.0, "weno5": 74.0}
+    if hyb:
+        h = np.array(flag_hist if flag_hist is not None else [1.0, 0.0, 0.0], dtype=float)
+        h = h / h.sum()
+        fl_rec = h[0] * rec["ud7"] + h[1] * rec["weno7"] + h[2] * rec["weno5"]
+    else:
+        fl_rec = rec[case.scheme]
+    inv_flops = 10 * fl_rec + 5 + 140 + 15
+    th = 8 if hyb else 0
+    m_inv = 32 if met3d else 0
+    out = {
+        "ghost_fill": (0.0, 0.0),
+        "primitives": (88.0 * P, 25.0 * P),
+        "shock_sensor": (16.0, 25.0),
+        "inviscid_x": (40 + th + m_inv + 40, inv_flops),
+        "inviscid_y": (40 + th + m_inv + 80, inv_flops),
+        "inviscid_z": (40 + th + m_inv + 80, inv_flops),
+        "viscous_flux": (32 + 96 + (80 if met3d else 0), 240.0),
+        "viscous_div": (96 + 64 + (8 if met3d else 0), 125.0),
+        "rk3_update": (160.0, 20.0),
+        "max_wavespeed": (40.0 + (80 if met3d else 0), 45.0),
+    }
+    return out
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU during the timed region (NVML)."""
+
+    def __init__(self, index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_steps(case, nsteps, warmup):
+    """Time the CPU oracle, as it stands, on `case`: returns (points*steps/s, seconds, threads)."""
+    from oracle.oracle import Oracle
+    o = Oracle(case)
+    U = o.fill_ghosts(case.U0.copy())
+    dt = case.cfl / o.max_wavespeed(U)
+    for _ in range(warmup):
+        o.rk3_step(U, dt)
+    t0 = time.perf_counter()
+    for _ in range(nsteps):
+        o.rk3_step(U, dt)
+    t = time.perf_counter() - t0
+    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return case.npoints * nsteps / t, t, threads
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    gen, twin, note = WORKLOADS[args.workload]
+    case = twin()
+    val, t, threads = oracle_steps(case, args.steps, min(args.warmup, 1))
+    sample = f"{case.name} twin of {args.workload}, {args.steps} RK3 steps, full oracle path"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "note": note, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2209_15333_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    gen, twin, note = WORKLOADS[args.workload]
+    t_gen = time.perf_counter()
+    case = gen()
+    t_gen = time.perf_counter() - t_gen
+    s = B.Solver(case, device=f"cuda:{local}")
+    U0_host = torch.from_numpy(case.U0)
+    U = U0_host.to(s.device)
+    s.fill_ghosts(U)
+    lam = s.max_wavespeed(U)
+    dt = case.cfl / lam
+    flag_hist = None
+    if case.scheme == "hybrid":
+        _, fl = s.debug_sensor(U)
+        flag_hist = torch.bincount(fl[fl < 3].flatten().to(torch.int64), minlength=3).cpu().numpy()
+        del fl
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        s.rk3_step(U, dt)
+    barrier()
+    # ---- timed region: K steps, CUDA events on the launch stream; per-kernel events inside the library
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s.timing(True)
+    n0 = s.launch_count()
+    with ClockSampler(local) as clk:
+        e0.record(s.stream)
+        for _ in range(args.steps):
+            s.rk3_step(U, dt)
+        e1.record(s.stream)
+        barrier()
+    ms = e0.elapsed_time(e1)
+    launches = s.launch_count() - n0
+    per_kernel = s.timing_read()
+    s.timing(False)
+    finite = bool(torch.isfinite(U).all().item())
+    tmax = torch.tensor([ms], dtype=torch.float64, device=s.device)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_all = float(tmax.item())
+    value = world * case.npoints * args.steps / (ms_all * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers: H2D + step + D2H inside the timed region, every step
+    n_e2e = max(1, min(args.steps, 3))
+    Uh = torch.empty(U0_host.shape, dtype=torch.float64, pin_memory=True)
+    Uh.copy_(U.cpu())
+    s.rk3_steps_host(Uh, U, dt, 1)          # warm-up of the copy path
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        s.rk3_steps_host(Uh, U, dt, 1)      # synchronises the stream before returning
+    barrier()
+    t_e2e = time.perf_counter() - t0
+    te = torch.tensor([t_e2e], dtype=torch.float64, device=s.device)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * case.npoints * n_e2e / float(te.item())
+    nbytes = int(Uh.numel() * 8)
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel, from the library's per-launch CUDA events over the timed region
+    hbm_peak, peak_src = peaks()
+    alg = algorithmic(case, flag_hist)
+    tot_kernel_ms = sum(v[0] for v in per_kernel.values())
+    kern = {}
+    for name, (kms, n) in per_kernel.items():
+        if n == 0:
+            continue
+        by, fl = alg[name]
+        per_launch_ms = kms / n
+        gbs = by * case.npoints / (per_launch_ms * 1e-3) / 1e9
+        tfl = fl * case.npoints / (per_launch_ms * 1e-3) / 1e12
+        kern[name] = {"ms_per_launch": per_launch_ms, "launches_per_step": n / args.steps, "share": kms / tot_kernel_ms,
+                      "alg_GBs": gbs, "alg_TFLOPs": tfl, "frac_hbm": gbs / hbm_peak, "frac_fp64": tfl / FP64_PEAK_TFLOPS}
+    top = max(kern, key=lambda k: kern[k]["share"])
+    kt = kern[top]
+    if kt["frac_fp64"] > kt["frac_hbm"]:
+        roof = {"kernel": top, "bound": "alu", "achieved": kt["alg_TFLOPs"], "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": kt["frac_fp64"], "peak_source": "fp64 DFMA probe (profiles/fp64_peak_r01.md)"}
+    else:
+        roof = {"kernel": top, "bound": "hbm", "achieved": kt["alg_GBs"], "peak": hbm_peak, "unit": "GB/s",
+                "frac": kt["frac_hbm"], "peak_source": f"MEASURED_PEAKS.json ({peak_src})"}
+    roof["traffic"] = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        try:
+            roof["traffic"] = json.load(open(tpath)).get(args.workload, {}).get(top)
+        except Exception:
+            pass
+
+    # ---- the oracle timed on this box's host cores, bounded sample of the same workload
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        tw = twin()
+        from oracle.oracle import Oracle  # noqa: F401  (cpu_baseline leg: the one place bench.py may run the oracle)
+        rate, _, threads = oracle_steps(tw, 1, 1)
+        nst = int(max(1, min(50, round(12.0 * rate / tw.npoints))))
+        rate, tsec, threads = oracle_steps(tw, nst, 0)
+        cpu = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"{tw.name} (twin of the workload, same generator), {nst} RK3 steps, {tsec:.1f} s"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_all / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "note": note, "grid": [case.nx, case.ny, case.nz], "points": case.npoints,
+                   "scheme": case.scheme, "grid_kind": case.grid_kind, "dt": dt, "cfl": case.cfl,
+                   "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
+                   "cache": "inputs larger than L2 (state 5 fields x %.0f MB)" % (np.prod(case.padded_shape) * 8 / 1e6),
+                   "hybrid_flag_hist_ud7_weno7_weno5": None if flag_hist is None else [int(v) for v in flag_hist],
+                   "input_generation_s": t_gen, "finite": finite},
+        "clocks": clk.summary(),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                "steps": n_e2e, "api": "ocfd_rk3_steps_host (pinned host buffer)"},
+        "gpu_launches": int(launches),
+        "roofline": roof,
+        "cpu_baseline": cpu,
+        "kernels": kern,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

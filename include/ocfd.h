@@ -122,6 +122,16 @@ ocfd_status ocfd_debug_sensor(ocfd_ctx *ctx, const double *U, double *theta, uns
 /* sizeof(ocfd_params) as compiled, so that a foreign-language mirror of the struct can check itself. */
 size_t ocfd_sizeof_params(void);
 
+/* Per-kernel-class device timing with CUDA events recorded on the launch stream around every kernel launch.
+ * ocfd_timing(ctx, 1) switches it on (and clears the record), ocfd_timing(ctx, 0) off.  ocfd_timing_read
+ * synchronises the stream, adds up the elapsed milliseconds and launch counts per class since the last read
+ * into ms[OCFD_NKERNELS] / launches[OCFD_NKERNELS] (host arrays) and clears the record.  Class names:
+ * ocfd_kernel_name(id), id = 0 .. OCFD_NKERNELS-1. */
+#define OCFD_NKERNELS 10
+ocfd_status ocfd_timing(ocfd_ctx *ctx, int enable);
+ocfd_status ocfd_timing_read(ocfd_ctx *ctx, double *ms, long long *launches);
+const char *ocfd_kernel_name(int id);
+
 /* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
 long long ocfd_launch_count(const ocfd_ctx *ctx);
 

@@ -17,8 +17,9 @@ BCS = {"periodic": 0, "wall": 1, "inflow": 2, "outflow": 3}
 OCFD_OK = 0
 
 EXPORTS = ["ocfd_workspace_bytes", "ocfd_init", "ocfd_destroy", "ocfd_fill_ghosts", "ocfd_rhs", "ocfd_rk3_step",
-           "ocfd_rk3_steps_host", "ocfd_max_wavespeed", "ocfd_debug_sensor", "ocfd_sizeof_params", "ocfd_launch_count",
-           "ocfd_strerror"]
+           "ocfd_rk3_steps_host", "ocfd_max_wavespeed", "ocfd_debug_sensor", "ocfd_timing", "ocfd_timing_read",
+           "ocfd_kernel_name", "ocfd_sizeof_params", "ocfd_launch_count", "ocfd_strerror"]
+NKERNELS = 10
 
 
 class OcfdParams(C.Structure):
@@ -80,6 +81,12 @@ def load():
     L.ocfd_launch_count.argtypes = [vp]
     L.ocfd_strerror.restype = C.c_char_p
     L.ocfd_strerror.argtypes = [C.c_int]
+    L.ocfd_timing.restype = C.c_int
+    L.ocfd_timing.argtypes = [vp, C.c_int]
+    L.ocfd_timing_read.restype = C.c_int
+    L.ocfd_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.ocfd_kernel_name.restype = C.c_char_p
+    L.ocfd_kernel_name.argtypes = [C.c_int]
     L.ocfd_sizeof_params.restype = C.c_size_t
     L.ocfd_sizeof_params.argtypes = []
     if L.ocfd_sizeof_params() != C.sizeof(OcfdParams):
@@ -219,6 +226,16 @@ class Solver:
         flags = self.torch.full((3,) + self.case_shape[1:], 255, dtype=self.torch.uint8, device=self.device)
         _check(self.L.ocfd_debug_sensor(self.ctx, self._ptr(U), theta.data_ptr(), flags.data_ptr()))
         return theta, flags
+
+    def timing(self, enable):
+        _check(self.L.ocfd_timing(self.ctx, 1 if enable else 0))
+
+    def timing_read(self):
+        """{kernel class name: (total ms, launches)} since the last read."""
+        ms = (C.c_double * NKERNELS)()
+        n = (C.c_longlong * NKERNELS)()
+        _check(self.L.ocfd_timing_read(self.ctx, ms, n))
+        return {self.L.ocfd_kernel_name(k).decode(): (ms[k], n[k]) for k in range(NKERNELS)}
 
     def launch_count(self):
         return int(self.L.ocfd_launch_count(self.ctx))

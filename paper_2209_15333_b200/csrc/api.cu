@@ -118,6 +118,8 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->scal = (double *)(w + cv.scal);
     c->flags = nullptr;
     c->launches = 0;
+    c->timing = 0;
+    c->tl_used = 0;
     *out = c;
     return OCFD_OK;
 }
@@ -125,6 +127,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
 ocfd_status ocfd_destroy(ocfd_ctx *c) {
     if (!live(c)) return OCFD_ESTATE;
     c->magic = 0;
+    for (auto &t : c->tl) { cudaEventDestroy(t.a); cudaEventDestroy(t.b); }
     delete c;
     return OCFD_OK;
 }
@@ -188,6 +191,35 @@ ocfd_status ocfd_debug_sensor(ocfd_ctx *c, const double *U, double *theta, unsig
         return OCFD_ECUDA;
     if (flag_xyz && (st = launch_flags(c, flag_xyz)) != OCFD_OK) return st;
     return OCFD_OK;
+}
+
+ocfd_status ocfd_timing(ocfd_ctx *c, int enable) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return OCFD_ECUDA;
+    c->timing = enable ? 1 : 0;
+    c->tl_used = 0;
+    return OCFD_OK;
+}
+
+ocfd_status ocfd_timing_read(ocfd_ctx *c, double *ms, long long *launches) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!ms || !launches) return OCFD_EINVAL;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return OCFD_ECUDA;
+    for (int k = 0; k < OCFD_NKERNELS; ++k) { ms[k] = 0.0; launches[k] = 0; }
+    for (size_t q = 0; q < c->tl_used; ++q) {
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, c->tl[q].a, c->tl[q].b) != cudaSuccess) return OCFD_ECUDA;
+        ms[c->tl[q].id] += t;
+        launches[c->tl[q].id]++;
+    }
+    c->tl_used = 0;
+    return OCFD_OK;
+}
+
+const char *ocfd_kernel_name(int id) {
+    static const char *names[OCFD_NKERNELS] = {"ghost_fill", "primitives", "shock_sensor", "inviscid_x", "inviscid_y",
+                                               "inviscid_z", "viscous_flux", "viscous_div", "rk3_update", "max_wavespeed"};
+    return id >= 0 && id < OCFD_NKERNELS ? names[id] : "?";
 }
 
 size_t ocfd_sizeof_params(void) { return sizeof(ocfd_params); }

@@ -120,6 +120,7 @@ ocfd_status launch_fill_ghosts(ocfd_ctx *c, double *U) {
             dim3 grd((F.n1 + blk.x - 1) / blk.x, (F.n2 + blk.y - 1) / blk.y, 1);
             if (pass == 0) {
                 if (bc != OCFD_BC_WALL_ISOTHERMAL && bc != OCFD_BC_SUPERSONIC_INFLOW) continue;
+                OCFD_T0(c, K_GHOST);
                 switch (g.kind) {
                     case OCFD_GRID_UNIFORM:
                         k_bc_nodes<OCFD_GRID_UNIFORM><<<grd, blk, 0, c->stream>>>(g, c->gas, F, bc, c->p.T_wall[f], c->p.wall_vn[f], c->p.inflow[f], U);
@@ -132,6 +133,7 @@ ocfd_status launch_fill_ghosts(ocfd_ctx *c, double *U) {
                 }
             } else {
                 grd.z = OCFD_NG;
+                OCFD_T0(c, K_GHOST);
                 k_bc_ghosts<<<grd, blk, 0, c->stream>>>(g, c->gas, F, bc, c->p.T_wall[f], c->p.inflow[f], U);
             }
             OCFD_CHECK_LAUNCH(c);

@@ -276,6 +276,7 @@ ocfd_status launch_kind_scheme(ocfd_ctx *c, const double *U, double *dU) {
     const GridDesc &g = c->g;
     {
         dim3 blk(XT, XL), grd((g.nx + XOUT - 1) / XOUT, (g.ny * g.nz + XL - 1) / XL);
+        OCFD_T0(c, K_INV_X);
         k_inviscid_x<KIND, SCHEME><<<grd, blk, 0, c->stream>>>(g, c->gas, U, c->prim, c->theta, dU);
         OCFD_CHECK_LAUNCH(c);
     }
@@ -288,11 +289,13 @@ ocfd_status launch_kind_scheme(ocfd_ctx *c, const double *U, double *dU) {
     }
     {
         dim3 blk(YW, YR), grd((g.nx + YW - 1) / YW, (g.ny + YS - 1) / YS, g.nz);
+        OCFD_T0(c, K_INV_Y);
         k_inviscid_yz<KIND, SCHEME, 1><<<grd, blk, shm, c->stream>>>(g, c->gas, U, c->prim, c->theta, dU);
         OCFD_CHECK_LAUNCH(c);
     }
     {
         dim3 blk(YW, YR), grd((g.nx + YW - 1) / YW, (g.nz + YS - 1) / YS, g.ny);
+        OCFD_T0(c, K_INV_Z);
         k_inviscid_yz<KIND, SCHEME, 2><<<grd, blk, shm, c->stream>>>(g, c->gas, U, c->prim, c->theta, dU);
         OCFD_CHECK_LAUNCH(c);
     }

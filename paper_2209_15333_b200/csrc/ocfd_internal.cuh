@@ -4,6 +4,8 @@
 #include <math.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "ocfd.h"
 
 #define OCFD_NG 4
@@ -32,6 +34,12 @@ struct GasDesc {
     double weno_eps, sw_eps, theta1, theta2;
 };
 
+// kernel classes, for ocfd_timing_read / ocfd_kernel_name
+enum { K_GHOST = 0, K_PRIM, K_SENSOR, K_INV_X, K_INV_Y, K_INV_Z, K_VISC_FLUX, K_VISC_DIV, K_RK, K_WAVE, K_COUNT };
+static_assert(K_COUNT == OCFD_NKERNELS, "kernel class count");
+
+struct TimedLaunch { cudaEvent_t a, b; int id; };
+
 struct ocfd_ctx {
     uint64_t magic;
     ocfd_params p;
@@ -47,7 +55,30 @@ struct ocfd_ctx {
     double *scal;    // small scalar area (wavespeed result)
     unsigned char *flags;  // [3][np] bytes (debug only)
     long long launches;
+    // optional per-launch timing with CUDA events on the launch stream (ocfd_timing)
+    int timing;
+    std::vector<TimedLaunch> tl;
+    size_t tl_used;
 };
+
+// bracket one kernel launch: OCFD_T0 before it, OCFD_CHECK_LAUNCH after it
+inline void ocfd_t0(ocfd_ctx *c, int id) {
+    if (!c->timing) return;
+    if (c->tl_used == c->tl.size()) {
+        TimedLaunch t;
+        cudaEventCreate(&t.a);
+        cudaEventCreate(&t.b);
+        c->tl.push_back(t);
+    }
+    c->tl[c->tl_used].id = id;
+    cudaEventRecord(c->tl[c->tl_used].a, c->stream);
+}
+inline void ocfd_t1(ocfd_ctx *c) {
+    if (!c->timing) return;
+    cudaEventRecord(c->tl[c->tl_used].b, c->stream);
+    c->tl_used++;
+}
+#define OCFD_T0(ctx, id) ocfd_t0((ctx), (id))
 
 // prim field order
 enum { P_U = 0, P_V = 1, P_W = 2, P_T = 3, P_C = 4, P_P = 5, P_NF = 6 };
@@ -97,6 +128,7 @@ ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
 
 #define OCFD_CHECK_LAUNCH(ctx)                                  \
     do {                                                        \
+        ocfd_t1(ctx);                                           \
         (ctx)->launches++;                                      \
         if (cudaGetLastError() != cudaSuccess) return OCFD_ECUDA; \
     } while (0)

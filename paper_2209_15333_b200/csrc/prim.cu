@@ -110,6 +110,7 @@ ocfd_status launch_prim(ocfd_ctx *c, const double *U) {
     long long np = c->g.np;
     int blocks = (int)((np + 255) / 256);
     if (blocks > 148 * 32) blocks = 148 * 32;
+    OCFD_T0(c, K_PRIM);
     k_prim<<<blocks, 256, 0, c->stream>>>(np, c->gas, U, c->prim);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
@@ -119,6 +120,7 @@ ocfd_status launch_sensor(ocfd_ctx *c, const double *U) {
     (void)U;
     const GridDesc &g = c->g;
     dim3 blk(32, 4, 2), grd((g.nx + 31) / 32, (g.ny + 3) / 4, (g.nz + 1) / 2);
+    OCFD_T0(c, K_SENSOR);
     k_sensor<<<grd, blk, 0, c->stream>>>(g, c->prim + (long long)P_P * g.np, c->theta);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
@@ -127,6 +129,7 @@ ocfd_status launch_sensor(ocfd_ctx *c, const double *U) {
 ocfd_status launch_flags(ocfd_ctx *c, unsigned char *flags) {
     const GridDesc &g = c->g;
     dim3 blk(32, 8, 1), grd((g.nxp + 31) / 32, (g.nyp + 7) / 8, g.nzp);
+    OCFD_T0(c, K_SENSOR);
     k_flags<<<grd, blk, 0, c->stream>>>(g, c->gas, (int)c->p.scheme, c->theta, flags);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
@@ -139,6 +142,7 @@ ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out) {
     long long n = (long long)g.nx * g.ny * g.nz;
     int blocks = (int)((n + 255) / 256);
     if (blocks > 148 * 16) blocks = 148 * 16;
+    OCFD_T0(c, K_WAVE);
     switch (g.kind) {
         case OCFD_GRID_UNIFORM: k_wavespeed<OCFD_GRID_UNIFORM><<<blocks, 256, 0, c->stream>>>(g, c->gas, U, out); break;
         case OCFD_GRID_STRETCHED: k_wavespeed<OCFD_GRID_STRETCHED><<<blocks, 256, 0, c->stream>>>(g, c->gas, U, out); break;

@@ -32,6 +32,7 @@ __global__ void __launch_bounds__(256) k_rk_update(GridDesc g, double *__restric
 ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage) {
     const GridDesc &g = c->g;
     dim3 blk(64, 4, 1), grd((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
+    OCFD_T0(c, K_RK);
     if (stage == 0) k_rk_update<0><<<grd, blk, 0, c->stream>>>(g, Un, U, dU, dt);
     else if (stage == 1) k_rk_update<1><<<grd, blk, 0, c->stream>>>(g, Un, U, dU, dt);
     else k_rk_update<2><<<grd, blk, 0, c->stream>>>(g, Un, U, dU, dt);

@@ -108,8 +108,10 @@ template <int KIND>
 ocfd_status launch_kind(ocfd_ctx *c, double *dU) {
     const GridDesc &g = c->g;
     dim3 blk(32, 4, 2), grd((g.nx + 31) / 32, (g.ny + 3) / 4, (g.nz + 1) / 2);
+    OCFD_T0(c, K_VISC_FLUX);
     k_viscous_flux<KIND><<<grd, blk, 0, c->stream>>>(g, c->gas, c->prim, c->Fv);
     OCFD_CHECK_LAUNCH(c);
+    OCFD_T0(c, K_VISC_DIV);
     k_viscous_div<KIND><<<grd, blk, 0, c->stream>>>(g, c->Fv, dU);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;

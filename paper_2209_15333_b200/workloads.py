@@ -343,8 +343,26 @@ def ramp(nx=2048, ny=300, nz=256, seed=20225, scheme="hybrid", theta2=np.inf, ns
     v = (um * sinw[None, :])[None] + sc * fl[1]
     w = sc * fl[2]
     del fl
-    T = np.broadcast_to(Tm[None], shp)
-    p = np.full(shp, pinf)
+    # the ramp's oblique shock (weak solution of the theta-beta-M relation for a 24 degree turn), smeared over
+    # about three cells with a tanh profile: it is what the shock sensor of the hybrid scheme has to find
+    turn = np.deg2rad(24.0)
+    lo, hi = np.arcsin(1.0 / Ma) + 1e-6, np.deg2rad(64.0)
+    for _ in range(100):
+        beta = 0.5 * (lo + hi)
+        tb = 2.0 / np.tan(beta) * (Ma ** 2 * np.sin(beta) ** 2 - 1.0) / (Ma ** 2 * (gamma + np.cos(2 * beta)) + 2.0)
+        lo, hi = (beta, hi) if tb < np.tan(turn) else (lo, beta)
+    m1n2 = (Ma * np.sin(beta)) ** 2
+    p_ratio = 1.0 + 2.0 * gamma / (gamma + 1.0) * (m1n2 - 1.0)
+    r_ratio = (gamma + 1.0) * m1n2 / ((gamma - 1.0) * m1n2 + 2.0)
+    v_ratio = np.sqrt(np.cos(beta) ** 2 + (np.sin(beta) / r_ratio) ** 2)
+    dsh = (np.tan(beta) * xs[None, :] - Y) * np.cos(beta)              # > 0 behind the shock
+    sh = 0.5 * (1.0 + np.tanh(dsh / (1.5 * dxx)))
+    fp_, ft_, fv_ = 1.0 + (p_ratio - 1.0) * sh, 1.0 + (p_ratio / r_ratio - 1.0) * sh, 1.0 + (v_ratio - 1.0) * sh
+    u *= fv_[None]
+    v *= fv_[None]
+    w *= fv_[None]
+    T = np.broadcast_to((Tm * ft_)[None], shp)
+    p = np.broadcast_to((pinf * fp_)[None], shp)
     rho = gamma * Ma * Ma * p / T
     U = cons_from_prim(rho, u, v, w, p, gamma)
     inflow = [None] * 6
