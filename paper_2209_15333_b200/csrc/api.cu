@@ -138,15 +138,21 @@ ocfd_status ocfd_fill_ghosts(ocfd_ctx *c, double *U) {
     return launch_fill_ghosts(c, U);
 }
 
-ocfd_status ocfd_rhs(ocfd_ctx *c, const double *U, double *dU) {
-    if (!live(c)) return OCFD_ESTATE;
-    if (!U || !dU || U == dU) return OCFD_EINVAL;
+// rows a2-a7; rk_stage >= 0 additionally folds the RK3 stage update (a8) into the last kernel that touches dU
+static ocfd_status rhs_impl(ocfd_ctx *c, double *U, double *dU, int rk_stage, double dt) {
     ocfd_status st;
     if ((st = launch_prim(c, U)) != OCFD_OK) return st;
     if (c->p.scheme == OCFD_HYBRID && (st = launch_sensor(c, U)) != OCFD_OK) return st;
     if ((st = launch_inviscid(c, U, dU)) != OCFD_OK) return st;
-    if (!c->p.inviscid && (st = launch_viscous(c, U, dU)) != OCFD_OK) return st;
+    if (!c->p.inviscid) return launch_viscous(c, dU, U, dt, rk_stage);
+    if (rk_stage >= 0) return launch_rk_update(c, c->Un, U, dU, dt, rk_stage);
     return OCFD_OK;
+}
+
+ocfd_status ocfd_rhs(ocfd_ctx *c, const double *U, double *dU) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U || !dU || U == dU) return OCFD_EINVAL;
+    return rhs_impl(c, const_cast<double *>(U), dU, -1, 0.0);  // rk_stage < 0: U is only read
 }
 
 ocfd_status ocfd_rk3_step(ocfd_ctx *c, double *U, double dt) {
@@ -155,8 +161,7 @@ ocfd_status ocfd_rk3_step(ocfd_ctx *c, double *U, double dt) {
     ocfd_status st;
     for (int s = 0; s < 3; ++s) {
         if ((st = launch_fill_ghosts(c, U)) != OCFD_OK) return st;
-        if ((st = ocfd_rhs(c, U, c->dUw)) != OCFD_OK) return st;
-        if ((st = launch_rk_update(c, c->Un, U, c->dUw, dt, s)) != OCFD_OK) return st;
+        if ((st = rhs_impl(c, U, c->dUw, s, dt)) != OCFD_OK) return st;
     }
     return launch_fill_ghosts(c, U);
 }

@@ -122,7 +122,7 @@ ocfd_status launch_prim(ocfd_ctx *c, const double *U);
 ocfd_status launch_sensor(ocfd_ctx *c, const double *U);
 ocfd_status launch_flags(ocfd_ctx *c, unsigned char *flags);
 ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU);
-ocfd_status launch_viscous(ocfd_ctx *c, const double *U, double *dU);
+ocfd_status launch_viscous(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage);
 ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage);
 ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
 
