@@ -15,6 +15,7 @@ bool valid_params(const ocfd_params *p) {
     if (!p) return false;
     if (p->ng != OCFD_NG) return false;
     if (p->nx < 8 || p->ny < 8 || p->nz < 8) return false;
+    if (p->nx % 2) return false;  // TMA: row pitch (nx+8)*8 bytes must be a multiple of 16
     if ((long long)(p->nx + 8) * (p->ny + 8) * (p->nz + 8) > (1ll << 40)) return false;
     if (!(p->gamma > 1.0) || !(p->Ma > 0.0) || !(p->weno_eps > 0.0) || !(p->sw_eps >= 0.0)) return false;
     if (!p->inviscid && (!(p->Re > 0.0) || !(p->Pr > 0.0) || !(p->T_ref > 0.0) || !(p->T_suth >= 0.0))) return false;
@@ -118,6 +119,10 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->scal = (double *)(w + cv.scal);
     c->flags = nullptr;
     c->launches = 0;
+    c->inv.ready = false;
+    c->inv.U = c->inv.dU = nullptr;
+    c->visc.ready = false;
+    c->visc.Up = c->visc.dUp = nullptr;
     c->timing = 0;
     c->tl_used = 0;
     *out = c;

@@ -1,5 +1,6 @@
 // Internal declarations shared by the CUDA translation units of libocfd_b200 (not part of the C ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -40,6 +41,19 @@ static_assert(K_COUNT == OCFD_NKERNELS, "kernel class count");
 
 struct TimedLaunch { cudaEvent_t a, b; int id; };
 
+// TMA tensor maps of the inviscid sweeps (per direction), re-encoded only when the caller's U / dU pointers change
+struct InvMaps {
+    const double *U, *dU;
+    bool ready;
+    CUtensorMap rho[3], prim[3], th[3], out[3];
+};
+// ... and of the two viscous passes
+struct ViscMaps {
+    const double *Up, *dUp;
+    bool ready;
+    CUtensorMap prim, F, G, H, dU, U, Un;
+};
+
 struct ocfd_ctx {
     uint64_t magic;
     ocfd_params p;
@@ -47,13 +61,15 @@ struct ocfd_ctx {
     GasDesc gas;
     cudaStream_t stream;
     // workspace carve-up (device pointers)
-    double *prim;    // [6][np]: u v w T c p
+    double *prim;    // [6][np]: T u v w c p
     double *theta;   // [np]
     double *Fv;      // [12][np]
     double *Un;      // [5][np]
     double *dUw;     // [5][np]
     double *scal;    // small scalar area (wavespeed result)
     unsigned char *flags;  // [3][np] bytes (debug only)
+    InvMaps inv;
+    ViscMaps visc;
     long long launches;
     // optional per-launch timing with CUDA events on the launch stream (ocfd_timing)
     int timing;
@@ -81,7 +97,8 @@ inline void ocfd_t1(ocfd_ctx *c) {
 #define OCFD_T0(ctx, id) ocfd_t0((ctx), (id))
 
 // prim field order
-enum { P_U = 0, P_V = 1, P_W = 2, P_T = 3, P_C = 4, P_P = 5, P_NF = 6 };
+// (T first and c after w: the viscous kernels fetch fields 0..3 = T,u,v,w, the inviscid sweeps 1..4 = u,v,w,c as one box)
+enum { P_T = 0, P_U = 1, P_V = 2, P_W = 3, P_C = 4, P_P = 5, P_NF = 6 };
 
 // ---------------------------------------------------------------- metric access
 // padded linear index of (ip,jp,kp)

@@ -3,15 +3,20 @@
 // points, pass 2 differences them and accumulates into dU (and, inside ocfd_rk3_step, applies the RK3 stage update
 // of eq. 45 in the same kernel so that dU is not written and re-read).
 //
-// Both passes are 2.5-D marching kernels: a block owns an x-y tile and walks along z.  Each thread keeps the seven
-// z-planes its zeta-derivative needs in registers, so every field value is fetched from HBM once; the x and y
-// neighbours of the current plane are exchanged through a shared-memory tile with 3-point halos.
+// Both passes are 2.5-D marching kernels: a CTA owns a 32 x 8 tile in x-y and walks along z.  Every z-plane of every
+// input is fetched exactly once, by TMA box loads into a ring of shared-memory stages that run two or more planes
+// ahead of the arithmetic (one elected thread issues them, completion is signalled on one mbarrier per stage), so the
+// HBM pipe stays full without tying up registers.  The seven z-planes the zeta-derivative needs live in a register
+// window per thread; the x / y neighbours of the current plane are read from the staged box (3-point halos; the box is
+// 4 wider in x on each side because a TMA box of doubles must start at an even x index).
 #include "ocfd_internal.cuh"
+#include "tma.cuh"
 
 namespace {
 
-constexpr int TX = 32, TY = 8;               // threads = tile of own points
-constexpr int SXW = TX + 6, SYW = TY + 6;    // shared tile with 3-point halos
+constexpr int TX = 32, TY = 8, VNT = TX * TY;  // own points of a tile = threads
+constexpr int BXW = TX + 8;                    // x extent of a box with x halos (i0-4 .. i0+TX+3)
+constexpr int BYH = TY + 6;                    // y extent of a box with y halos (j0-3 .. j0+TY+2)
 
 __device__ __forceinline__ double d1c(double m3, double m2, double m1, double p1, double p2, double p3) {
     return (45.0 * (p1 - m1) - 9.0 * (p2 - m2) + (p3 - m3)) * (1.0 / 60.0);
@@ -34,208 +39,295 @@ __device__ __forceinline__ double d1_line(const double *p, int st, int s, int n,
     return (8.0 * (p[st] - p[-st]) - (p[2 * st] - p[-2 * st])) * (1.0 / 12.0);
 }
 
-__device__ __forceinline__ int clampi(int v, int lo, int hi) { return v < lo ? lo : (v > hi ? hi : v); }
-__device__ __forceinline__ int wrapi(int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); }
-
 // ------------------------------------------------------------------------------------------------ a6
-// prim: padded fields u,v,w,T (valid on interior + face ghosts).  Fv: [12][np], written at interior points.
+// Input: primitive fields 0..3 = T,u,v,w (valid on interior + face ghosts).  Output Fv[12][np] at interior points,
+// plus, on periodic axes, the three image planes each direction's flux needs beyond the faces (pass 2 fetches plain
+// boxes and cannot wrap).
+constexpr int VF_NST = 6;                       // ring: planes k..k+3 live, two more in flight
+constexpr int VF_STAGE = 4 * BYH * BXW;         // doubles per stage
+constexpr size_t VF_SMEM = sizeof(double) * VF_NST * VF_STAGE + 8 * VF_NST;
+
 template <int KIND>
-__global__ void __launch_bounds__(TX *TY, 2) k_viscous_flux(GridDesc g, GasDesc gs, const double *__restrict__ prim,
-                                                         double *__restrict__ Fv, int zchunk) {
-    __shared__ double sp[4][SYW][SXW];
+__global__ void __launch_bounds__(VNT, 2)
+    k_viscous_flux(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_prim,
+                   const double *__restrict__ prim, double *__restrict__ Fv, int zchunk) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *ring = reinterpret_cast<double *>(smem_raw);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(ring + VF_NST * VF_STAGE);
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
     const int i = i0 + tx, j = j0 + ty;
     const bool own = i < g.nx && j < g.ny;
-    // threads past the ragged edge still stage their (ghost) column: the last own points differentiate through it
-    const int ip = min(i, g.nx + OCFD_NG - 1) + OCFD_NG, jp = min(j, g.ny + OCFD_NG - 1) + OCFD_NG;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
-    const long long col = (long long)jp * g.sy + ip;  // padded offset within a plane
-    // z window: planes k-3 .. k+3 of the four fields at this thread's column
+    const int last = k1 + 2;  // last plane the window needs
+    auto issue = [&](int plane) {  // plane k (interior index) -> stage (k - k0) % NST
+        const int s = (plane - k0) % VF_NST;
+        tma::mbar_expect_tx(&bars[s], VF_STAGE * 8);
+        tma::load4(ring + s * VF_STAGE, &tm_prim, &bars[s], i0, j0 + 1, plane + OCFD_NG, 0);
+    };
+    if (tid == 0) {
+        for (int s = 0; s < VF_NST; ++s) tma::mbar_init(&bars[s], 1);
+        tma::fence_barrier_init();
+        for (int q = 0; q < VF_NST; ++q)
+            if (k0 + q <= last) issue(k0 + q);
+    }
+    // z window: planes k-3 .. k+3 of T,u,v,w at this thread's column.  The three planes below the chunk come
+    // straight from global memory, everything else through the ring.
+    const int ipc = min(i, g.nx - 1) + OCFD_NG, jpc = min(j, g.ny - 1) + OCFD_NG;
+    const long long col = (long long)jpc * g.sy + ipc;
+    const int ctr = (ty + 3) * BXW + tx + 4;  // own point inside a staged field
     double w[4][7];
 #pragma unroll
     for (int a = 0; a < 4; ++a)
 #pragma unroll
-        for (int q = 0; q < 6; ++q) w[a][q + 1] = prim[a * g.np + (long long)(k0 - 3 + q + OCFD_NG) * g.sz + col];
-    // metrics of this column are needed every step; for z-extruded grids they do not depend on k
+        for (int q = 0; q < 3; ++q) w[a][q + 1] = __ldg(prim + a * g.np + (long long)(k0 - 3 + q + OCFD_NG) * g.sz + col);
+    __syncthreads();  // barriers initialised
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        tma::mbar_wait(&bars[q], 0);
+#pragma unroll
+        for (int a = 0; a < 4; ++a) w[a][q + 4] = ring[q * VF_STAGE + a * BYH * BXW + ctr];
+    }
     for (int k = k0; k < k1; ++k) {
         const int kp = k + OCFD_NG;
+        const int sn = (k + 3 - k0) % VF_NST;
+        tma::mbar_wait(&bars[sn], ((k + 3 - k0) / VF_NST) & 1);
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
 #pragma unroll
             for (int q = 0; q < 6; ++q) w[a][q] = w[a][q + 1];
-            w[a][6] = prim[a * g.np + (long long)(kp + 3) * g.sz + col];
+            w[a][6] = ring[sn * VF_STAGE + a * BYH * BXW + ctr];
         }
-        __syncthreads();  // previous plane's tile is no longer read
+        if (own) {
+            const double *sp = ring + ((k - k0) % VF_NST) * VF_STAGE + ctr;
+            double gr[4][3];
 #pragma unroll
-        for (int a = 0; a < 4; ++a) sp[a][ty + 3][tx + 3] = w[a][3];
-        // halo cells of plane k (x: 2x3 columns, y: 2x3 rows; corners are not needed)
-        for (int c = tid; c < 2 * 3 * TY + 2 * 3 * TX; c += TX * TY) {
-            int hx, hy;
-            if (c < 6 * TY) { hx = (c % 6 < 3) ? c % 6 : TX + c % 6; hy = 3 + c / 6; }
-            else { const int e = c - 6 * TY; hx = 3 + e % TX; hy = (e / TX < 3) ? e / TX : TY + e / TX; }
-            const int gi = clampi(i0 - 3 + hx, -OCFD_NG, g.nx + OCFD_NG - 1) + OCFD_NG;
-            const int gj = clampi(j0 - 3 + hy, -OCFD_NG, g.ny + OCFD_NG - 1) + OCFD_NG;
-            const long long id = (long long)kp * g.sz + (long long)gj * g.sy + gi;
+            for (int a = 0; a < 4; ++a) {
+                gr[a][0] = d1_line(sp + a * BYH * BXW, 1, i, g.nx, g.periodic[0]);
+                gr[a][1] = d1_line(sp + a * BYH * BXW, BXW, j, g.ny, g.periodic[1]);
+                gr[a][2] = d1_seven(w[a], k, g.nz, g.periodic[2]);
+            }
+            const int ip = i + OCFD_NG, jp = j + OCFD_NG;
+            double m[3][3];
 #pragma unroll
-            for (int a = 0; a < 4; ++a) sp[a][hy][hx] = __ldg(prim + a * g.np + id);
+            for (int d = 0; d < 3; ++d) Met<KIND>::row(g, d, ip, jp, kp, m[d][0], m[d][1], m[d][2]);
+            const double iJ = 1.0 / Met<KIND>::J(g, ip, jp, kp);
+            double gx[4], gy[4], gz[4];  // Cartesian gradients of T,u,v,w (chain rule)
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                gx[a] = m[0][0] * gr[a][0] + m[1][0] * gr[a][1] + m[2][0] * gr[a][2];
+                gy[a] = m[0][1] * gr[a][0] + m[1][1] * gr[a][1] + m[2][1] * gr[a][2];
+                gz[a] = m[0][2] * gr[a][0] + m[1][2] * gr[a][1] + m[2][2] * gr[a][2];
+            }
+            const double T = w[0][3], u = w[1][3], v = w[2][3], ww = w[3][3];
+            const double mu0 = (1.0 + gs.suth) / (T + gs.suth) * T * sqrt(T);  // eq. 15
+            const double mu = mu0 * gs.invRe, kc = mu0 * gs.kfac;              // eq. 14
+            const double div = gx[1] + gy[2] + gz[3];
+            const double txx = mu * (2.0 * gx[1] - (2.0 / 3.0) * div);         // eq. 13
+            const double tyy = mu * (2.0 * gy[2] - (2.0 / 3.0) * div);
+            const double tzz = mu * (2.0 * gz[3] - (2.0 / 3.0) * div);
+            const double txy = mu * (gy[1] + gx[2]), txz = mu * (gz[1] + gx[3]), tyz = mu * (gz[2] + gy[3]);
+            const double thx = u * txx + v * txy + ww * txz + kc * gx[0];      // eq. 12 (R-2)
+            const double thy = u * txy + v * tyy + ww * tyz + kc * gy[0];
+            const double thz = u * txz + v * tyz + ww * tzz + kc * gz[0];
+            const long long id = (long long)kp * g.sz + (long long)jp * g.sy + ip;
+            const int c[3] = {i, j, k}, n[3] = {g.nx, g.ny, g.nz};
+            const long long st[3] = {1, g.sy, g.sz};
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {                                       // eq. 9-11
+                const double dx = m[d][0] * iJ, dy = m[d][1] * iJ, dz = m[d][2] * iJ;
+                const double f0 = dx * txx + dy * txy + dz * txz, f1 = dx * txy + dy * tyy + dz * tyz;
+                const double f2 = dx * txz + dy * tyz + dz * tzz, f3 = dx * thx + dy * thy + dz * thz;
+                double *F = Fv + (4 * d) * g.np;
+                F[id] = f0; F[g.np + id] = f1; F[2 * g.np + id] = f2; F[3 * g.np + id] = f3;
+                if (g.periodic[d]) {  // images beyond the faces of this direction's own axis
+                    long long im = -1;
+                    if (c[d] < 3) im = id + n[d] * st[d];
+                    else if (c[d] >= n[d] - 3) im = id - n[d] * st[d];
+                    if (im >= 0) { F[im] = f0; F[g.np + im] = f1; F[2 * g.np + im] = f2; F[3 * g.np + im] = f3; }
+                }
+            }
         }
-        __syncthreads();
-        if (!own) continue;
-        double gr[4][3];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            gr[a][0] = d1_line(&sp[a][ty + 3][tx + 3], 1, i, g.nx, g.periodic[0]);
-            gr[a][1] = d1_line(&sp[a][ty + 3][tx + 3], SXW, j, g.ny, g.periodic[1]);
-            gr[a][2] = d1_seven(w[a], k, g.nz, g.periodic[2]);
-        }
-        double m[3][3];
-#pragma unroll
-        for (int d = 0; d < 3; ++d) Met<KIND>::row(g, d, ip, jp, kp, m[d][0], m[d][1], m[d][2]);
-        const double iJ = 1.0 / Met<KIND>::J(g, ip, jp, kp);
-        double gx[4], gy[4], gz[4];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {  // chain rule
-            gx[a] = m[0][0] * gr[a][0] + m[1][0] * gr[a][1] + m[2][0] * gr[a][2];
-            gy[a] = m[0][1] * gr[a][0] + m[1][1] * gr[a][1] + m[2][1] * gr[a][2];
-            gz[a] = m[0][2] * gr[a][0] + m[1][2] * gr[a][1] + m[2][2] * gr[a][2];
-        }
-        const double u = w[0][3], v = w[1][3], ww = w[2][3], T = w[3][3];
-        const double mu0 = (1.0 + gs.suth) / (T + gs.suth) * T * sqrt(T);  // eq. 15
-        const double mu = mu0 * gs.invRe, kc = mu0 * gs.kfac;              // eq. 14
-        const double div = gx[0] + gy[1] + gz[2];
-        const double txx = mu * (2.0 * gx[0] - (2.0 / 3.0) * div);         // eq. 13
-        const double tyy = mu * (2.0 * gy[1] - (2.0 / 3.0) * div);
-        const double tzz = mu * (2.0 * gz[2] - (2.0 / 3.0) * div);
-        const double txy = mu * (gy[0] + gx[1]), txz = mu * (gz[0] + gx[2]), tyz = mu * (gz[1] + gy[2]);
-        const double thx = u * txx + v * txy + ww * txz + kc * gx[3];      // eq. 12 (R-2)
-        const double thy = u * txy + v * tyy + ww * tyz + kc * gy[3];
-        const double thz = u * txz + v * tyz + ww * tzz + kc * gz[3];
-        const long long id = (long long)kp * g.sz + col;
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {                                       // eq. 9-11
-            const double dx = m[d][0] * iJ, dy = m[d][1] * iJ, dz = m[d][2] * iJ;
-            Fv[(4 * d + 0) * g.np + id] = dx * txx + dy * txy + dz * txz;
-            Fv[(4 * d + 1) * g.np + id] = dx * txy + dy * tyy + dz * tyz;
-            Fv[(4 * d + 2) * g.np + id] = dx * txz + dy * tyz + dz * tzz;
-            Fv[(4 * d + 3) * g.np + id] = dx * thx + dy * thy + dz * thz;
-        }
+        __syncthreads();  // every thread is done with plane k: its stage can be refilled
+        if (tid == 0 && k + VF_NST <= last) issue(k + VF_NST);
     }
 }
 
 // ------------------------------------------------------------------------------------------------ a7 (+ a8)
 // RK: 0 = plain accumulate into dU (ocfd_rhs); 1..3 = also apply RK3 stage RK-1 (eq. 45) to U, dU is not written.
+// One stage holds, for plane k: F with x halos, G with y halos, dU, U, U^n of the tile, and H of plane k+3.
+constexpr int VD_NST = 3;
+constexpr int VD_F = 4 * TY * BXW, VD_G = 4 * BYH * TX, VD_H = 4 * TY * TX, VD_C = 5 * TY * TX;
+constexpr int VD_STAGE = VD_F + VD_G + VD_H + 3 * VD_C;
+constexpr size_t VD_SMEM = sizeof(double) * VD_NST * VD_STAGE + 8 * VD_NST;
+static_assert((VD_F * 8) % 128 == 0 && (VD_G * 8) % 128 == 0 && (VD_H * 8) % 128 == 0 && (VD_C * 8) % 128 == 0 &&
+              (VD_STAGE * 8) % 128 == 0 && (VF_STAGE * 8) % 128 == 0, "TMA destinations must stay 128-byte aligned");
+
 template <int KIND, int RK>
-__global__ void __launch_bounds__(TX *TY, 2) k_viscous_div(GridDesc g, const double *__restrict__ Fv, double *__restrict__ dU,
-                                                        double *__restrict__ U, double *__restrict__ Un, double dt,
-                                                        int zchunk) {
-    __shared__ double sF[4][TY][SXW];   // xi-direction flux with x halos
-    __shared__ double sG[4][SYW][TX];   // eta-direction flux with y halos
+__global__ void __launch_bounds__(VNT, 1)
+    k_viscous_div(const GridDesc g, const __grid_constant__ CUtensorMap tm_F, const __grid_constant__ CUtensorMap tm_G,
+                  const __grid_constant__ CUtensorMap tm_H, const __grid_constant__ CUtensorMap tm_dU,
+                  const __grid_constant__ CUtensorMap tm_U, const __grid_constant__ CUtensorMap tm_Un,
+                  const double *__restrict__ Fv, double *__restrict__ dU, double *__restrict__ U,
+                  double *__restrict__ Un, double dt, int zchunk) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *ring = reinterpret_cast<double *>(smem_raw);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(ring + VD_NST * VD_STAGE);
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
     const int i = i0 + tx, j = j0 + ty;
     const bool own = i < g.nx && j < g.ny;
-    const int ip = (own ? i : g.nx - 1) + OCFD_NG, jp = (own ? j : g.ny - 1) + OCFD_NG;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
-    const long long col = (long long)jp * g.sy + ip;
-    const double *H = Fv + 8 * g.np;
-    // z window of the zeta-direction flux: interior planes only; periodic axes wrap, aperiodic ones never read outside
-    auto zplane = [&](int k) -> long long {
-        const int kk = g.periodic[2] ? wrapi(k, g.nz) : clampi(k, 0, g.nz - 1);
-        return (long long)(kk + OCFD_NG) * g.sz;
+    constexpr bool LD_U = RK != 0, LD_UN = RK >= 2;
+    constexpr uint32_t BYTES = 8u * (VD_F + VD_G + VD_H + VD_C + (LD_U ? VD_C : 0) + (LD_UN ? VD_C : 0));
+    auto issue = [&](int k) {
+        const int s = (k - k0) % VD_NST;
+        double *b = ring + s * VD_STAGE;
+        const int xp = i0 + OCFD_NG, yp = j0 + OCFD_NG, kp = k + OCFD_NG;
+        tma::mbar_expect_tx(&bars[s], BYTES);
+        tma::load4(b, &tm_F, &bars[s], xp - 4, yp, kp, 0);
+        tma::load4(b + VD_F, &tm_G, &bars[s], xp, yp - 3, kp, 4);
+        tma::load4(b + VD_F + VD_G, &tm_H, &bars[s], xp, yp, kp + 3, 8);
+        tma::load4(b + VD_F + VD_G + VD_H, &tm_dU, &bars[s], xp, yp, kp, 0);
+        if (LD_U) tma::load4(b + VD_F + VD_G + VD_H + VD_C, &tm_U, &bars[s], xp, yp, kp, 0);
+        if (LD_UN) tma::load4(b + VD_F + VD_G + VD_H + 2 * VD_C, &tm_Un, &bars[s], xp, yp, kp, 0);
     };
+    if (tid == 0) {
+        for (int s = 0; s < VD_NST; ++s) tma::mbar_init(&bars[s], 1);
+        tma::fence_barrier_init();
+        for (int q = 0; q < VD_NST; ++q)
+            if (k0 + q < k1) issue(k0 + q);
+    }
+    // z window of the zeta-direction flux H: planes k-3 .. k+2 from global memory, plane k+3 arrives with stage k
+    const int ipc = min(i, g.nx - 1) + OCFD_NG, jpc = min(j, g.ny - 1) + OCFD_NG;
+    const long long col = (long long)jpc * g.sy + ipc;
+    const double *H = Fv + 8 * g.np;
     double w[4][7];
 #pragma unroll
     for (int r = 0; r < 4; ++r)
 #pragma unroll
-        for (int q = 0; q < 6; ++q) w[r][q + 1] = H[r * g.np + zplane(k0 - 3 + q) + col];
+        for (int q = 0; q < 6; ++q) w[r][q + 1] = __ldg(H + r * g.np + (long long)(k0 - 3 + q + OCFD_NG) * g.sz + col);
+    __syncthreads();  // barriers initialised
+    const int ctr = ty * TX + tx;
     for (int k = k0; k < k1; ++k) {
-        const int kp = k + OCFD_NG;
-        const long long pl = (long long)kp * g.sz;
+        const int s = (k - k0) % VD_NST;
+        const double *b = ring + s * VD_STAGE;
+        tma::mbar_wait(&bars[s], ((k - k0) / VD_NST) & 1);
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
 #pragma unroll
             for (int q = 0; q < 6; ++q) w[r][q] = w[r][q + 1];
-            w[r][6] = H[r * g.np + zplane(k + 3) + col];
+            w[r][6] = b[VD_F + VD_G + r * TY * TX + ctr];
         }
-        __syncthreads();
-        // own values + halos of F (x) and G (y) for plane k
-        for (int c = tid; c < TY * SXW; c += TX * TY) {
-            const int hx = c % SXW, hy = c / SXW;
-            int gi = i0 - 3 + hx;
-            gi = g.periodic[0] ? wrapi(gi, g.nx) : clampi(gi, 0, g.nx - 1);
-            const int gj = min(j0 + hy, g.ny - 1);
-            const long long id = pl + (long long)(gj + OCFD_NG) * g.sy + gi + OCFD_NG;
+        if (own) {
+            const int ip = i + OCFD_NG, jp = j + OCFD_NG, kp = k + OCFD_NG;
+            const long long id = (long long)kp * g.sz + (long long)jp * g.sy + ip;
+            const double J = Met<KIND>::J(g, ip, jp, kp);
+            const double *sdU = b + VD_F + VD_G + VD_H, *sU = sdU + VD_C, *sUn = sU + VD_C;
+            double acc[5];
+            acc[0] = sdU[ctr];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) sF[r][hy][hx] = __ldg(Fv + r * g.np + id);
-        }
-        for (int c = tid; c < SYW * TX; c += TX * TY) {
-            const int hx = c % TX, hy = c / TX;
-            int gj = j0 - 3 + hy;
-            gj = g.periodic[1] ? wrapi(gj, g.ny) : clampi(gj, 0, g.ny - 1);
-            const int gi = min(i0 + hx, g.nx - 1);
-            const long long id = pl + (long long)(gj + OCFD_NG) * g.sy + gi + OCFD_NG;
+            for (int r = 0; r < 4; ++r) {
+                double sum = d1_line(b + (r * TY + ty) * BXW + tx + 4, 1, i, g.nx, g.periodic[0]);
+                sum += d1_line(b + VD_F + (r * BYH + ty + 3) * TX + tx, TX, j, g.ny, g.periodic[1]);
+                sum += d1_seven(w[r], k, g.nz, g.periodic[2]);
+                acc[r + 1] = sdU[(r + 1) * TY * TX + ctr] + J * sum;
+            }
+            if (RK == 0) {
 #pragma unroll
-            for (int r = 0; r < 4; ++r) sG[r][hy][hx] = __ldg(Fv + (4 + r) * g.np + id);
-        }
-        __syncthreads();
-        if (!own) continue;
-        const long long id = pl + col;
-        const double J = Met<KIND>::J(g, ip, jp, kp);
-        double acc[5];
-        acc[0] = dU[id];
+                for (int r = 1; r < 5; ++r) dU[r * g.np + id] = acc[r];
+            } else {
 #pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            // interior stencils wrap through the staged halos, so "periodic" is passed as 1 only when the axis is
-            double s = d1_line(&sF[r][ty][tx + 3], 1, i, g.nx, g.periodic[0]);
-            s += d1_line(&sG[r][ty + 3][tx], TX, j, g.ny, g.periodic[1]);
-            s += d1_seven(w[r], k, g.nz, g.periodic[2]);
-            acc[r + 1] = dU[(r + 1) * g.np + id] + J * s;
-        }
-        if (RK == 0) {
-#pragma unroll
-            for (int r = 1; r < 5; ++r) dU[r * g.np + id] = acc[r];
-        } else {
-#pragma unroll
-            for (int m = 0; m < 5; ++m) {
-                const long long q = m * g.np + id;
-                const double u = U[q];
-                if (RK == 1) {
-                    Un[q] = u;
-                    U[q] = u + dt * acc[m];
-                } else if (RK == 2) {
-                    U[q] = 0.75 * Un[q] + 0.25 * (u + dt * acc[m]);
-                } else {
-                    U[q] = (1.0 / 3.0) * Un[q] + (2.0 / 3.0) * (u + dt * acc[m]);
+                for (int m = 0; m < 5; ++m) {
+                    const long long q = m * g.np + id;
+                    const double u = sU[m * TY * TX + ctr];
+                    if (RK == 1) {
+                        Un[q] = u;
+                        U[q] = u + dt * acc[m];
+                    } else if (RK == 2) {
+                        U[q] = 0.75 * sUn[m * TY * TX + ctr] + 0.25 * (u + dt * acc[m]);
+                    } else {
+                        U[q] = (1.0 / 3.0) * sUn[m * TY * TX + ctr] + (2.0 / 3.0) * (u + dt * acc[m]);
+                    }
                 }
             }
         }
+        __syncthreads();  // stage s is free again
+        if (tid == 0 && k + VD_NST < k1) issue(k + VD_NST);
     }
 }
 
 int pick_zchunk(const GridDesc &g) {
-    // enough blocks to fill 148 SMs a few times over, chunks long enough that the 6 halo planes stay cheap
+    // enough blocks to fill 148 SMs a few times over, chunks long enough that the prologue planes stay cheap
     const long long tiles = (long long)((g.nx + TX - 1) / TX) * ((g.ny + TY - 1) / TY);
     int zc = g.nz;
     while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < 148 * 8) zc = (zc + 1) / 2;
     return zc;
 }
 
+bool encode_maps(ocfd_ctx *c, const double *dU, const double *U) {
+    const GridDesc &g = c->g;
+    ViscMaps &M = c->visc;
+    const long long d6[4] = {g.nxp, g.nyp, g.nzp, P_NF}, d12[4] = {g.nxp, g.nyp, g.nzp, 12}, d5[4] = {g.nxp, g.nyp, g.nzp, 5};
+    const int bp[4] = {BXW, BYH, 1, 4}, bF[4] = {BXW, TY, 1, 4}, bG[4] = {TX, BYH, 1, 4}, bH[4] = {TX, TY, 1, 4};
+    const int bC[4] = {TX, TY, 1, 5};
+    if (!M.ready) {
+        if (!ocfd_tma_encode(&M.prim, c->prim, d6, g.sy, g.sz, g.np, bp)) return false;
+        if (!ocfd_tma_encode(&M.F, c->Fv, d12, g.sy, g.sz, g.np, bF)) return false;
+        if (!ocfd_tma_encode(&M.G, c->Fv, d12, g.sy, g.sz, g.np, bG)) return false;
+        if (!ocfd_tma_encode(&M.H, c->Fv, d12, g.sy, g.sz, g.np, bH)) return false;
+        if (!ocfd_tma_encode(&M.Un, c->Un, d5, g.sy, g.sz, g.np, bC)) return false;
+        M.ready = true;
+    }
+    if (M.dUp != dU) {
+        if (!ocfd_tma_encode(&M.dU, dU, d5, g.sy, g.sz, g.np, bC)) return false;
+        M.dUp = dU;
+    }
+    if (U && M.Up != U) {
+        if (!ocfd_tma_encode(&M.U, U, d5, g.sy, g.sz, g.np, bC)) return false;
+        M.Up = U;
+    }
+    return true;
+}
+
+template <int KIND, int RK>
+ocfd_status launch_div(ocfd_ctx *c, dim3 grd, dim3 blk, double *dU, double *U, double dt, int zc) {
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_viscous_div<KIND, RK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VD_SMEM) != cudaSuccess)
+            return OCFD_ECUDA;
+        attr_set = true;
+    }
+    const ViscMaps &M = c->visc;
+    k_viscous_div<KIND, RK><<<grd, blk, VD_SMEM, c->stream>>>(c->g, M.F, M.G, M.H, M.dU, RK ? M.U : M.dU, M.Un, c->Fv, dU, U,
+                                                             c->Un, dt, zc);
+    return OCFD_OK;
+}
+
 template <int KIND>
 ocfd_status launch_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
     const GridDesc &g = c->g;
+    if (!encode_maps(c, dU, rk_stage >= 0 ? U : nullptr)) return OCFD_ECUDA;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_viscous_flux<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VF_SMEM) != cudaSuccess)
+            return OCFD_ECUDA;
+        attr_set = true;
+    }
     const int zc = pick_zchunk(g);
     dim3 blk(TX, TY, 1), grd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zc - 1) / zc);
     OCFD_T0(c, K_VISC_FLUX);
-    k_viscous_flux<KIND><<<grd, blk, 0, c->stream>>>(g, c->gas, c->prim, c->Fv, zc);
+    k_viscous_flux<KIND><<<grd, blk, VF_SMEM, c->stream>>>(g, c->gas, c->visc.prim, c->prim, c->Fv, zc);
     OCFD_CHECK_LAUNCH(c);
     OCFD_T0(c, K_VISC_DIV);
+    ocfd_status st;
     switch (rk_stage) {
-        case 0: k_viscous_div<KIND, 1><<<grd, blk, 0, c->stream>>>(g, c->Fv, dU, U, c->Un, dt, zc); break;
-        case 1: k_viscous_div<KIND, 2><<<grd, blk, 0, c->stream>>>(g, c->Fv, dU, U, c->Un, dt, zc); break;
-        case 2: k_viscous_div<KIND, 3><<<grd, blk, 0, c->stream>>>(g, c->Fv, dU, U, c->Un, dt, zc); break;
-        default: k_viscous_div<KIND, 0><<<grd, blk, 0, c->stream>>>(g, c->Fv, dU, nullptr, nullptr, 0.0, zc);
+        case 0: st = launch_div<KIND, 1>(c, grd, blk, dU, U, dt, zc); break;
+        case 1: st = launch_div<KIND, 2>(c, grd, blk, dU, U, dt, zc); break;
+        case 2: st = launch_div<KIND, 3>(c, grd, blk, dU, U, dt, zc); break;
+        default: st = launch_div<KIND, 0>(c, grd, blk, dU, nullptr, 0.0, zc);
     }
+    if (st != OCFD_OK) return st;
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
