@@ -78,15 +78,18 @@ def algorithmic(case, flag_hist=None):
     inv_flops = 10 * fl_rec + 5 + 140 + 15
     th = 8 if hyb else 0
     m_inv = 32 if met3d else 0
+    state = 8 + 32                      # rho from U, (u,v,w,c) from the primitive fields
     out = {
         "ghost_fill": (0.0, 0.0),
         "primitives": (88.0 * P, 25.0 * P),
         "shock_sensor": (16.0, 25.0),
-        "inviscid_x": (40 + th + m_inv + 40, inv_flops),
-        "inviscid_y": (40 + th + m_inv + 80, inv_flops),
-        "inviscid_z": (40 + th + m_inv + 80, inv_flops),
+        # x sweep writes dU; y / z sweeps add into it (TMA reduce at the L2: dU still crosses HBM in and out)
+        "inviscid_x": (state + th + m_inv + 40, inv_flops),
+        "inviscid_y": (state + th + m_inv + 80, inv_flops),
+        "inviscid_z": (state + th + m_inv + 80, inv_flops),
         "viscous_flux": (32 + 96 + (80 if met3d else 0), 240.0),
-        "viscous_div": (96 + 64 + (8 if met3d else 0), 125.0),
+        # a7 + a8 fused (inside ocfd_rk3_step): R Fv 96 + dU 40 + U 40 + U^n 40 (W at stage 1), W U 40
+        "viscous_div": (96 + 40 + 40 + 40 + 40 + (8 if met3d else 0), 125.0 + 20.0),
         "rk3_update": (160.0, 20.0),
         "max_wavespeed": (40.0 + (80 if met3d else 0), 45.0),
     }

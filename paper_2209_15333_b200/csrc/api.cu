@@ -45,7 +45,7 @@ bool valid_params(const ocfd_params *p) {
     return true;
 }
 
-struct Carve { size_t prim, theta, Fv, Un, dUw, scal, total; };
+struct Carve { size_t prim, theta, Fv, Un, dUw, scal, mtab, total; };
 
 Carve carve(const ocfd_params *p) {
     const size_t np = (size_t)(p->nx + 8) * (p->ny + 8) * (p->nz + 8);
@@ -58,6 +58,13 @@ Carve carve(const ocfd_params *p) {
     c.Un = off; off += align_up(5 * np * sizeof(double), 256);
     c.dUw = off; off += align_up(5 * np * sizeof(double), 256);
     c.scal = off; off += 256;
+    c.mtab = off;
+    if (p->grid_kind == OCFD_GRID_CURVILINEAR) {
+        const size_t planes = p->metric_plane_stride ? (size_t)(p->nz + 8) : 1;
+        off += align_up(12 * planes * (size_t)(p->nx + 8) * (p->ny + 8) * sizeof(double), 256);
+    } else if (p->grid_kind == OCFD_GRID_STRETCHED) {
+        off += align_up((size_t)(p->nx + p->ny + p->nz + 24) * sizeof(double), 256);
+    }
     c.total = off;
     return c;
 }
@@ -117,6 +124,17 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->Un = (double *)(w + cv.Un);
     c->dUw = (double *)(w + cv.dUw);
     c->scal = (double *)(w + cv.scal);
+    c->mtab = (double *)(w + cv.mtab);
+    for (int d = 0; d < 3; ++d) { g.atab[d] = nullptr; g.rmet[d] = nullptr; g.ua[d] = 0.0; }
+    g.atab_fs = 0;
+    if (p->grid_kind == OCFD_GRID_UNIFORM) {
+        g.ua[0] = g.ux / g.uJ; g.ua[1] = g.uy / g.uJ; g.ua[2] = g.uz / g.uJ;
+    } else if (p->grid_kind == OCFD_GRID_STRETCHED) {
+        g.rmet[0] = c->mtab; g.rmet[1] = c->mtab + g.nxp; g.rmet[2] = c->mtab + g.nxp + g.nyp;
+    } else {
+        g.atab_fs = (g.msk ? (long long)g.nzp : 1ll) * g.sz;
+        for (int d = 0; d < 3; ++d) g.atab[d] = c->mtab + 4 * d * g.atab_fs;
+    }
     c->flags = nullptr;
     c->launches = 0;
     c->inv.ready = false;
@@ -125,6 +143,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->visc.Up = c->visc.dUp = nullptr;
     c->timing = 0;
     c->tl_used = 0;
+    if (launch_metric_tables(c) != OCFD_OK) { delete c; return OCFD_ECUDA; }
     *out = c;
     return OCFD_OK;
 }

@@ -22,6 +22,14 @@ struct GridDesc {
     double ux, uy, uz;     // uniform: 1/dx, 1/dy, 1/dz
     double uJ;             // uniform: J
     int periodic[3];
+    // derived metric data built once at init (launch_metric_tables), so that no kernel divides by J per point:
+    //   curvilinear: atab[d] = [4][planes][nyp][nxp] fields (d_x/J, d_y/J, d_z/J, J), k-plane stride msk (0 if extruded)
+    //   stretched:   rmet[d] = 1-D arrays 1/xi_x(i), 1/eta_y(j), 1/zeta_z(k)
+    //   uniform:     ua[d] = dx dy dz / spacing of axis d  (= d_d/J)
+    const double *atab[3];
+    long long atab_fs;     // field stride of atab (doubles)
+    const double *rmet[3];
+    double ua[3];
 };
 
 // Gas / scheme constants handed to kernels by value.
@@ -67,6 +75,7 @@ struct ocfd_ctx {
     double *Un;      // [5][np]
     double *dUw;     // [5][np]
     double *scal;    // small scalar area (wavespeed result)
+    double *mtab;    // derived metric tables (see GridDesc)
     unsigned char *flags;  // [3][np] bytes (debug only)
     InvMaps inv;
     ViscMaps visc;
@@ -133,7 +142,32 @@ struct Met {
     }
 };
 
+// Contravariant metric row of direction DIR divided by J (alpha of eq. 20-22) and J itself at a padded point.
+template <int KIND, int DIR>
+__device__ __forceinline__ void met_alpha(const GridDesc &g, int ip, int jp, int kp, double &a1, double &a2, double &a3,
+                                          double &J) {
+    if (KIND == OCFD_GRID_UNIFORM) {
+        a1 = DIR == 0 ? g.ua[0] : 0.0;
+        a2 = DIR == 1 ? g.ua[1] : 0.0;
+        a3 = DIR == 2 ? g.ua[2] : 0.0;
+        J = g.uJ;
+    } else if (KIND == OCFD_GRID_STRETCHED) {
+        const double rx = __ldg(g.rmet[0] + ip), ry = __ldg(g.rmet[1] + jp), rz = __ldg(g.rmet[2] + kp);
+        a1 = DIR == 0 ? ry * rz : 0.0;
+        a2 = DIR == 1 ? rx * rz : 0.0;
+        a3 = DIR == 2 ? rx * ry : 0.0;
+        J = (__ldg(g.met[0] + ip) * __ldg(g.met[4] + jp)) * __ldg(g.met[8] + kp);
+    } else {
+        const double *t = g.atab[DIR] + (long long)kp * g.msk + (long long)jp * g.sy + ip;
+        a1 = __ldg(t);
+        a2 = __ldg(t + g.atab_fs);
+        a3 = __ldg(t + 2 * g.atab_fs);
+        J = __ldg(t + 3 * g.atab_fs);
+    }
+}
+
 // ---------------------------------------------------------------- kernel launchers (host side)
+ocfd_status launch_metric_tables(ocfd_ctx *c);
 ocfd_status launch_fill_ghosts(ocfd_ctx *c, double *U);
 ocfd_status launch_prim(ocfd_ctx *c, const double *U);
 ocfd_status launch_sensor(ocfd_ctx *c, const double *U);
