@@ -61,7 +61,7 @@ Carve carve(const ocfd_params *p) {
     c.mtab = off;
     if (p->grid_kind == OCFD_GRID_CURVILINEAR) {
         const size_t planes = p->metric_plane_stride ? (size_t)(p->nz + 8) : 1;
-        off += align_up(12 * planes * (size_t)(p->nx + 8) * (p->ny + 8) * sizeof(double), 256);
+        off += align_up(15 * planes * (size_t)(p->nx + 8) * (p->ny + 8) * sizeof(double), 256);
     } else if (p->grid_kind == OCFD_GRID_STRETCHED) {
         off += align_up((size_t)(p->nx + p->ny + p->nz + 24) * sizeof(double), 256);
     }
@@ -90,11 +90,14 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     if (cudaGetDevice(&dev) != cudaSuccess) return OCFD_ECUDA;
     if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return OCFD_ECUDA;
     if (major < 10) return OCFD_EUNSUPPORTED;  // sm_100a only; there is no other code path
+    int nsm = 0;
+    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) return OCFD_ECUDA;
     ocfd_ctx *c = new (std::nothrow) ocfd_ctx();
     if (!c) return OCFD_EINVAL;
     c->magic = kMagic;
     c->p = *p;
     c->stream = (cudaStream_t)p->stream;
+    c->nsm = nsm;
     GridDesc &g = c->g;
     g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
     g.nxp = p->nx + 8; g.nyp = p->ny + 8; g.nzp = p->nz + 8;
@@ -112,6 +115,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     s.gamma = p->gamma; s.gm1 = p->gamma - 1.0; s.Ma = p->Ma; s.gM2 = p->gamma * p->Ma * p->Ma; s.invMa = 1.0 / p->Ma;
     s.inv2g = 1.0 / (2.0 * p->gamma);
     s.w0 = (3.0 - p->gamma) / (2.0 * (p->gamma - 1.0));
+    s.w1 = s.w0 + 0.5;
     s.tgm1 = 2.0 * (p->gamma - 1.0);
     s.suth = p->inviscid ? 0.0 : p->T_suth / p->T_ref;
     s.invRe = p->inviscid ? 0.0 : 1.0 / p->Re;
@@ -133,12 +137,14 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
         g.rmet[0] = c->mtab; g.rmet[1] = c->mtab + g.nxp; g.rmet[2] = c->mtab + g.nxp + g.nyp;
     } else {
         g.atab_fs = (g.msk ? (long long)g.nzp : 1ll) * g.sz;
-        for (int d = 0; d < 3; ++d) g.atab[d] = c->mtab + 4 * d * g.atab_fs;
+        for (int d = 0; d < 3; ++d) g.atab[d] = c->mtab + 5 * d * g.atab_fs;
     }
     c->flags = nullptr;
     c->launches = 0;
     c->inv.ready = false;
     c->inv.U = c->inv.dU = nullptr;
+    c->march.ready = false;
+    c->march.U = c->march.dU = nullptr;
     c->visc.ready = false;
     c->visc.Up = c->visc.dUp = nullptr;
     c->timing = 0;

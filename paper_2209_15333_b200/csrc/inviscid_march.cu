@@ -1,0 +1,312 @@
+// Rows a4 + a5 for the y and z sweeps: Steger-Warming split (eq. 19-29), UD7 / WENO7 / WENO5
+// reconstruction (eq. 41) and the conservative flux difference, as a MARCHING kernel.
+//
+// A CTA owns MAC = 32 pencils (32 consecutive x) of one cross index and walks along the sweep direction through all
+// nd + 8 padded rows in chunks of MR = 4 rows.  Every chunk:
+//   TMA      the state of the chunk (rho from U; u,v,w,c from the primitive fields; theta if hybrid) arrives in a ring
+//            of MNST = 3 stages that runs two chunks ahead of the arithmetic (one mbarrier per stage);
+//   phase A  one thread per point of the chunk: split fluxes f+-[5] -> shared memory.  Each point is split exactly
+//            once per sweep (no halo recomputation) and f+- never reach HBM (the paper materialises them, L549);
+//   phase B  one thread per (pencil, component): the 7-point windows of f+ and f- live in registers for the whole
+//            march, each new row costs two shared-memory loads; h_{i+1/2} is formed as soon as row i+4 has been
+//            pushed and -J (h_{i+1/2} - h_{i-1/2}) goes to an output tile in shared memory;
+//   TMA      the output tile leaves by one reduce-add per chunk (dU += at the L2; the x sweep has written dU before).
+// The output tensor map covers the interior of dU only, so the rows before the first interior point, ragged tiles and
+// ghosts are clipped by the hardware.
+#include "ocfd_internal.cuh"
+#include "schemes.cuh"
+#include "tma.cuh"
+
+#include <type_traits>
+
+namespace {
+
+constexpr int MAC = 32;             // pencils per CTA (consecutive x)
+constexpr int MR = 4;               // rows per chunk
+constexpr int MNST = 3;             // input stages
+constexpr int MPTS = MAC * MR;      // points per chunk
+constexpr int MNT = 5 * MAC;        // threads: one walker per (pencil, component)
+constexpr int MSTG = 6 * MPTS;      // doubles per input stage: rho, u, v, w, c, theta
+constexpr size_t M_SMEM = sizeof(double) * (size_t)(MNST * MSTG + 10 * MPTS + 2 * 5 * MPTS) + 8 * MNST + 4 * MAC;
+static_assert(MPTS <= MNT && (MPTS * 8) % 128 == 0, "chunk shape");
+
+// J along one pencil of the sweep: at(g, i0, e) = J at padded row i0 + e
+template <int KIND, int DIR>
+struct JRow {
+    const double *p;   // curvilinear: J of row 0 of the pencil; stretched: the 1-D metric of the sweep axis
+    long long st;      // curvilinear: row stride
+    double f0, f1;     // stretched: the two fixed 1-D metrics
+    __device__ __forceinline__ JRow(const GridDesc &g, int ip, int crossp) : p(nullptr), st(0), f0(0.0), f1(0.0) {
+        if (KIND == OCFD_GRID_STRETCHED) {
+            f0 = __ldg(g.met[0] + ip);
+            f1 = __ldg(g.met[DIR == 1 ? 8 : 4] + crossp);
+            p = g.met[DIR == 1 ? 4 : 8];
+        } else if (KIND == OCFD_GRID_CURVILINEAR) {
+            st = DIR == 1 ? g.sy : g.msk;
+            p = g.atab[0] + 4 * g.atab_fs + (DIR == 1 ? (long long)crossp * g.msk : (long long)crossp * g.sy) + ip;
+        }
+    }
+    __device__ __forceinline__ double at(const GridDesc &g, int i0, int e) const {
+        if (KIND == OCFD_GRID_UNIFORM) return g.uJ;
+        if (KIND == OCFD_GRID_STRETCHED) {
+            const double m = __ldg(p + i0 + e);
+            return DIR == 1 ? (f0 * m) * f1 : (f0 * f1) * m;   // (xi_x eta_y) zeta_z
+        }
+        return __ldg(p + (long long)(i0 + e) * st);
+    }
+};
+
+// h_{i+1/2} = recon(f+ window) + recon(mirrored f- window); out of line for the hybrid scheme (rare path, one copy)
+template <int SCHEME>
+__device__ __noinline__ double recon_pair_slow(int flag, double p0, double p1, double p2, double p3, double p4, double p5,
+                                               double p6, double m0, double m1, double m2, double m3, double m4, double m5,
+                                               double m6, double eps) {
+    return recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps) + recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
+}
+template <int SCHEME>
+__device__ __forceinline__ double recon_pair(int flag, double p0, double p1, double p2, double p3, double p4, double p5,
+                                             double p6, double m0, double m1, double m2, double m3, double m4, double m5,
+                                             double m6, double eps) {
+    if (SCHEME == OCFD_HYBRID) return recon_pair_slow<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, m0, m1, m2, m3, m4, m5, m6, eps);
+    return recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps) + recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
+}
+
+// KIND: grid kind, SCHEME: ocfd_scheme, DIR: 1 y, 2 z.  grid = (tiles across x, cross extent)
+template <int KIND, int SCHEME, int DIR>
+__global__ void __launch_bounds__(MNT, 4)
+    k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
+                     const __grid_constant__ CUtensorMap tm_prim, const __grid_constant__ CUtensorMap tm_th,
+                     const __grid_constant__ CUtensorMap tm_out) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *sIn = reinterpret_cast<double *>(smem_raw);   // [MNST][6][MR][MAC]
+    double *sF = sIn + MNST * MSTG;                       // [10][MR][MAC]: f+ (0..4), f- (5..9) of the current chunk
+    double *sO = sF + 10 * MPTS;                          // [2][5][MR][MAC] output tiles
+    uint64_t *bars = reinterpret_cast<uint64_t *>(sO + 2 * 5 * MPTS);
+    unsigned char *sFl = reinterpret_cast<unsigned char *>(bars + MNST);   // [MAC][MR] scheme flags pf of the chunk
+
+    const int tid = threadIdx.x;
+    const int a0 = blockIdx.x * MAC, cross = blockIdx.y;
+    const int nd = DIR == 1 ? g.ny : g.nz;
+    const int ndp = nd + 2 * OCFD_NG;
+    const int nch = (ndp + MR - 1) / MR;
+
+    auto issue = [&](int c) {   // one thread: boxes of chunk c (padded rows MR*c ..) towards stage c % MNST
+        const int s = c % MNST;
+        double *dst = sIn + s * MSTG;
+        const int c0 = OCFD_NG + a0;
+        const int c1 = DIR == 1 ? MR * c : OCFD_NG + cross;
+        const int c2 = DIR == 2 ? MR * c : OCFD_NG + cross;
+        tma::mbar_expect_tx(&bars[s], (SCHEME == OCFD_HYBRID ? 6 : 5) * MPTS * 8);
+        tma::load4(dst, &tm_rho, &bars[s], c0, c1, c2, 0);
+        tma::load4(dst + MPTS, &tm_prim, &bars[s], c0, c1, c2, P_U);
+        if (SCHEME == OCFD_HYBRID) tma::load4(dst + 5 * MPTS, &tm_th, &bars[s], c0, c1, c2, 0);
+    };
+    if (tid == 0) {
+#pragma unroll
+        for (int q = 0; q < MNST; ++q) tma::mbar_init(&bars[q], 1);
+        tma::fence_barrier_init();
+        issue(0);
+        if (nch > 1) issue(1);
+    }
+
+    // phase A role: point (row pr, pencil pa) of every chunk; walker role: pencil wa, component wm
+    const int pr = tid / MAC, pa = tid % MAC;
+    const bool producer = tid < MPTS;
+    const int wa = pa, wm = pr;
+    const int ipA = OCFD_NG + a0 + pa;
+    const bool x_ok = ipA < g.nxp - OCFD_NG;   // pencils past the last interior x hold zero-filled state
+    const JRow<KIND, DIR> jrow(g, min(ipA, g.nxp - 1), OCFD_NG + cross);
+
+    // Register windows as rings of 8: padded row r lives in slot r % 8.  Two chunks (8 rows) bring every slot back to
+    // its place, so the chunk loop is unrolled by two and no value is ever moved between registers.
+    double Wp[8], Wm[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) Wp[e] = Wm[e] = 0.0;
+    double hprev = 0.0;
+    unsigned pprev = 0;     // packed scheme flags pf(r) of the previous chunk's rows, 2 bits per row (hybrid)
+    __syncthreads();        // barriers initialised before anyone polls them
+
+    // one chunk; PH = c % 2 fixes the ring slots at compile time
+    auto chunk = [&](const int c, auto ph) {
+        constexpr int PH = decltype(ph)::value;
+        const int s = c % MNST;
+        const double *sU = sIn + s * MSTG;
+        const int r0 = MR * c;   // first padded row of the chunk
+
+        // metric data, fetched while the boxes are in flight: k, sigma of this thread's point (phase A) ...
+        double k1 = 0.0, k2 = 0.0, k3 = 0.0, sig = 1.0, Jdead;
+        const int rowA = r0 + pr;
+        const bool validA = producer && x_ok && rowA < ndp;
+        if (validA)
+            met_ksJ<KIND, DIR>(g, ipA, DIR == 1 ? rowA : OCFD_NG + cross, DIR == 2 ? rowA : OCFD_NG + cross, k1, k2, k3, sig,
+                               Jdead);
+        // ... and J of the four points this walker completes in this chunk (padded rows r0-4 .. r0-1; the first
+        // chunk completes nothing that is kept)
+        double Jw[MR];
+        {
+            const int i0 = max(r0 - OCFD_NG, 0);
+#pragma unroll
+            for (int e = 0; e < MR; ++e) Jw[e] = jrow.at(g, i0, e);
+        }
+        tma::mbar_wait(&bars[s], (c / MNST) & 1);
+
+        // ---- phase A: split fluxes of the chunk's points; pf(r) = scheme flag of the interface between rows r-1, r
+        if (producer) {
+            double *dst = sF + tid;
+            if (validA) {
+                sw_split_store<KIND, DIR>(gs, sU[tid], sU[MPTS + tid], sU[2 * MPTS + tid], sU[3 * MPTS + tid],
+                                          sU[4 * MPTS + tid], k1, k2, k3, sig, dst, MPTS);
+            } else {
+#pragma unroll
+                for (int q = 0; q < 10; ++q) dst[q * MPTS] = 0.0;
+            }
+            if (SCHEME == OCFD_HYBRID) {
+                unsigned char f = 0;
+                if (rowA >= OCFD_NG && rowA <= nd + OCFD_NG) {   // interfaces -1/2 .. nd-1/2 (eq. 42, R-12)
+                    const double *thp = pr > 0 ? sU + 5 * MPTS + tid - MAC
+                                               : sIn + ((c + MNST - 1) % MNST) * MSTG + 5 * MPTS + (MR - 1) * MAC + pa;
+                    f = (unsigned char)iface_flag(gs, *thp, sU[5 * MPTS + tid]);
+                }
+                sFl[4 * pa + pr] = f;
+            }
+        }
+        __syncthreads();
+        // the stage of chunk c-1 is free now (phase A of this chunk read its last theta row)
+        if (tid == 0 && c + 2 < nch && c > 0) issue(c + 2);
+
+        // ---- phase B: push the chunk's rows through the register windows
+        // pushing row r completes interface (r-4)+1/2 (f+ rows r-7..r-1, f- rows r-6..r) and with it point r-4
+        double *so = sO + PH * 5 * MPTS + wm * MPTS + wa;
+        const double *fpn = sF + wm * MPTS + wa, *fmn = sF + (wm + 5) * MPTS + wa;
+        bool fast = SCHEME == OCFD_UD7;
+        unsigned cur = 0;
+        if (SCHEME == OCFD_HYBRID) {
+            const unsigned w = reinterpret_cast<const unsigned *>(sFl)[wa];
+            const unsigned pc = (w & 3u) | ((w >> 6) & 0xcu) | ((w >> 12) & 0x30u) | ((w >> 18) & 0xc0u);
+            // the interfaces completed in this chunk: pf(r0-3), pf(r0-2), pf(r0-1), pf(r0)
+            cur = ((pprev >> 2) | (pc << 6)) & 0xffu;
+            pprev = pc;
+            fast = cur == 0;
+        }
+        double nP[MR], nM[MR];   // the chunk's new rows (loaded up front, entered into the rings one by one)
+#pragma unroll
+        for (int e = 0; e < MR; ++e) {
+            nP[e] = fpn[e * MAC];
+            nM[e] = fmn[e * MAC];
+        }
+        if (fast) {
+#pragma unroll
+            for (int e = 0; e < MR; ++e) {
+                const int k = 4 * PH + e;
+                Wp[k & 7] = nP[e];
+                Wm[k & 7] = nM[e];
+                const double h = ud7(Wp[(k + 1) & 7], Wp[(k + 2) & 7], Wp[(k + 3) & 7], Wp[(k + 4) & 7], Wp[(k + 5) & 7],
+                                     Wp[(k + 6) & 7], Wp[(k + 7) & 7]) +
+                                 ud7(Wm[k & 7], Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
+                                     Wm[(k + 3) & 7], Wm[(k + 2) & 7]);
+                so[e * MAC] = -Jw[e] * (h - hprev);
+                hprev = h;
+            }
+        } else {
+#pragma unroll
+            for (int e = 0; e < MR; ++e) {
+                const int k = 4 * PH + e;
+                Wp[k & 7] = nP[e];
+                Wm[k & 7] = nM[e];
+                const int flag = SCHEME == OCFD_HYBRID ? (int)((cur >> (2 * e)) & 3u) : 0;
+                const double h = recon_pair<SCHEME>(flag, Wp[(k + 1) & 7], Wp[(k + 2) & 7], Wp[(k + 3) & 7], Wp[(k + 4) & 7],
+                                                    Wp[(k + 5) & 7], Wp[(k + 6) & 7], Wp[(k + 7) & 7], Wm[k & 7],
+                                                    Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
+                                                    Wm[(k + 3) & 7], Wm[(k + 2) & 7], gs.weno_eps);
+                so[e * MAC] = -Jw[e] * (h - hprev);
+                hprev = h;
+            }
+        }
+        tma::fence_proxy_async();
+        __syncthreads();
+        if (tid == 0 && r0 + MR - 1 >= 2 * OCFD_NG) {
+            const int o = r0 - 2 * OCFD_NG;   // interior index of the first completed point (negative rows are clipped)
+            tma::reduce_add4(&tm_out, sO + PH * 5 * MPTS, a0, DIR == 1 ? o : cross, DIR == 2 ? o : cross, 0);
+            tma::store_commit();
+            tma::store_wait_read<1>();   // the other output tile is free for the next chunk
+        }
+    };
+    if (tid == 0 && nch > 2) issue(2);
+    for (int c = 0; c < nch; c += 2) {
+        chunk(c, std::integral_constant<int, 0>());
+        if (c + 1 < nch) chunk(c + 1, std::integral_constant<int, 1>());
+    }
+    if (tid == 0) tma::store_wait_all<0>();
+}
+
+template <int KIND, int SCHEME, int DIR>
+ocfd_status launch_march(ocfd_ctx *c) {
+    const GridDesc &g = c->g;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_inviscid_march<KIND, SCHEME, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)M_SMEM) != cudaSuccess)
+            return OCFD_ECUDA;
+        attr_set = true;
+    }
+    const int ncross = DIR == 1 ? g.nz : g.ny;
+    if (ncross > 65535) return OCFD_EINVAL;
+    dim3 grd((g.nx + MAC - 1) / MAC, ncross, 1);
+    OCFD_T0(c, K_INV_X + DIR);
+    const MarchMaps &M = c->march;
+    k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.rho[DIR], M.prim[DIR], M.th[DIR],
+                                                                        M.out[DIR]);
+    OCFD_CHECK_LAUNCH(c);
+    return OCFD_OK;
+}
+
+template <int KIND, int SCHEME>
+ocfd_status launch_march_dir(ocfd_ctx *c, int dir) {
+    return dir == 1 ? launch_march<KIND, SCHEME, 1>(c) : launch_march<KIND, SCHEME, 2>(c);
+}
+
+template <int KIND>
+ocfd_status launch_march_kind(ocfd_ctx *c, int dir) {
+    switch (c->p.scheme) {
+        case OCFD_UD7: return launch_march_dir<KIND, OCFD_UD7>(c, dir);
+        case OCFD_WENO7: return launch_march_dir<KIND, OCFD_WENO7>(c, dir);
+        case OCFD_WENO5: return launch_march_dir<KIND, OCFD_WENO5>(c, dir);
+        default: return launch_march_dir<KIND, OCFD_HYBRID>(c, dir);
+    }
+}
+
+// input boxes over the whole padded arrays, output boxes over the interior of dU
+bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
+    const GridDesc &g = c->g;
+    MarchMaps &M = c->march;
+    const long long full1[4] = {g.nxp, g.nyp, g.nzp, 1}, full6[4] = {g.nxp, g.nyp, g.nzp, P_NF};
+    const long long inner[4] = {g.nx, g.ny, g.nz, 5};
+    for (int d = 1; d < 3; ++d) {
+        const int by = d == 1 ? MR : 1, bz = d == 2 ? MR : 1;
+        const int b1[4] = {MAC, by, bz, 1}, b4[4] = {MAC, by, bz, 4}, bo[4] = {MAC, by, bz, 5};
+        if (!M.ready) {
+            if (!ocfd_tma_encode(&M.prim[d], c->prim, full6, g.sy, g.sz, g.np, b4)) return false;
+            if (!ocfd_tma_encode(&M.th[d], c->theta, full1, g.sy, g.sz, g.np, b1)) return false;
+        }
+        if (M.U != U && !ocfd_tma_encode(&M.rho[d], U, full1, g.sy, g.sz, g.np, b1)) return false;
+        if (M.dU != dU &&
+            !ocfd_tma_encode(&M.out[d], dU + (long long)OCFD_NG * (g.sz + g.sy + 1), inner, g.sy, g.sz, g.np, bo))
+            return false;
+    }
+    M.ready = true;
+    M.U = U;
+    M.dU = dU;
+    return true;
+}
+
+}  // namespace
+
+ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int dir) {
+    if (dir != 1 && dir != 2) return OCFD_EINVAL;
+    if (!encode_march_maps(c, U, dU)) return OCFD_ECUDA;
+    switch (c->g.kind) {
+        case OCFD_GRID_UNIFORM: return launch_march_kind<OCFD_GRID_UNIFORM>(c, dir);
+        case OCFD_GRID_STRETCHED: return launch_march_kind<OCFD_GRID_STRETCHED>(c, dir);
+        default: return launch_march_kind<OCFD_GRID_CURVILINEAR>(c, dir);
+    }
+}

@@ -1,5 +1,6 @@
-// Derived metric data, built once per context (ocfd_init): alpha_d = (d_x, d_y, d_z)/J of eq. 20-22 (PAPER.md:L161-
-// 176) for curvilinear grids, reciprocal 1-D spacings for stretched grids.  The sweeps then never divide by J.
+// Derived metric data, built once per context (ocfd_init): for curvilinear grids sigma = |alpha_d| and the unit normal
+// k_d = alpha_d/sigma of alpha_d = (d_x, d_y, d_z)/J (eq. 20-22); reciprocal 1-D spacings for
+// stretched grids.  The sweeps then never divide nor take a square root for the metrics.
 #include "ocfd_internal.cuh"
 
 namespace {
@@ -10,11 +11,14 @@ __global__ void k_alpha_tables(GridDesc g, double *__restrict__ tab, long long n
         const double J = g.met[9][id];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            double *t = tab + 4 * d * g.atab_fs + id;
-            t[0] = g.met[3 * d][id] / J;
-            t[g.atab_fs] = g.met[3 * d + 1][id] / J;
-            t[2 * g.atab_fs] = g.met[3 * d + 2][id] / J;
-            t[3 * g.atab_fs] = J;
+            double *t = tab + 5 * d * g.atab_fs + id;
+            const double a1 = g.met[3 * d][id] / J, a2 = g.met[3 * d + 1][id] / J, a3 = g.met[3 * d + 2][id] / J;
+            const double sigma = sqrt(a1 * a1 + a2 * a2 + a3 * a3);
+            t[0] = a1 / sigma;
+            t[g.atab_fs] = a2 / sigma;
+            t[2 * g.atab_fs] = a3 / sigma;
+            t[3 * g.atab_fs] = sigma;
+            t[4 * g.atab_fs] = J;
         }
     }
 }

@@ -23,7 +23,8 @@ struct GridDesc {
     double uJ;             // uniform: J
     int periodic[3];
     // derived metric data built once at init (launch_metric_tables), so that no kernel divides by J per point:
-    //   curvilinear: atab[d] = [4][planes][nyp][nxp] fields (d_x/J, d_y/J, d_z/J, J), k-plane stride msk (0 if extruded)
+    //   curvilinear: atab[d] = [5][planes][nyp][nxp] fields (k1, k2, k3, sigma, J) with alpha = (d_x, d_y, d_z)/J,
+    //                sigma = |alpha|, k = alpha/sigma; k-plane stride msk (0 if extruded)
     //   stretched:   rmet[d] = 1-D arrays 1/xi_x(i), 1/eta_y(j), 1/zeta_z(k)
     //   uniform:     ua[d] = dx dy dz / spacing of axis d  (= d_d/J)
     const double *atab[3];
@@ -37,6 +38,7 @@ struct GasDesc {
     double gamma, gm1, Ma, gM2, invMa;  // gM2 = gamma Ma^2
     double inv2g;                       // 1/(2 gamma)
     double w0;                          // (3-gamma)/(2(gamma-1))   (eq. 26)
+    double w1;                          // w0 + 1/2
     double tgm1;                        // 2(gamma-1)
     double suth;                        // T_suth/T_ref
     double invRe, kfac;                 // 1/Re, 1/((gamma-1) Ma^2 Pr Re)
@@ -55,6 +57,12 @@ struct InvMaps {
     bool ready;
     CUtensorMap rho[3], prim[3], th[3], out[3];
 };
+// ... of the marching sweeps (inviscid_march.cu), same roles, other box shapes
+struct MarchMaps {
+    const double *U, *dU;
+    bool ready;
+    CUtensorMap rho[3], prim[3], th[3], out[3];
+};
 // ... and of the two viscous passes
 struct ViscMaps {
     const double *Up, *dUp;
@@ -68,6 +76,7 @@ struct ocfd_ctx {
     GridDesc g;
     GasDesc gas;
     cudaStream_t stream;
+    int nsm;         // SM count of the device (persistent kernels launch a multiple of it)
     // workspace carve-up (device pointers)
     double *prim;    // [6][np]: T u v w c p
     double *theta;   // [np]
@@ -78,6 +87,7 @@ struct ocfd_ctx {
     double *mtab;    // derived metric tables (see GridDesc)
     unsigned char *flags;  // [3][np] bytes (debug only)
     InvMaps inv;
+    MarchMaps march;
     ViscMaps visc;
     long long launches;
     // optional per-launch timing with CUDA events on the launch stream (ocfd_timing)
@@ -142,27 +152,35 @@ struct Met {
     }
 };
 
-// Contravariant metric row of direction DIR divided by J (alpha of eq. 20-22) and J itself at a padded point.
+// Unit normal k = alpha/|alpha| and length sigma = |alpha| of alpha = (d_x, d_y, d_z)/J (eq. 20-22) of direction DIR,
+// and J itself, at a padded point.
 template <int KIND, int DIR>
-__device__ __forceinline__ void met_alpha(const GridDesc &g, int ip, int jp, int kp, double &a1, double &a2, double &a3,
-                                          double &J) {
+__device__ __forceinline__ void met_ksJ(const GridDesc &g, int ip, int jp, int kp, double &k1, double &k2, double &k3,
+                                        double &sigma, double &J) {
     if (KIND == OCFD_GRID_UNIFORM) {
-        a1 = DIR == 0 ? g.ua[0] : 0.0;
-        a2 = DIR == 1 ? g.ua[1] : 0.0;
-        a3 = DIR == 2 ? g.ua[2] : 0.0;
+        const double a = g.ua[DIR];
+        const double sg = a < 0.0 ? -1.0 : 1.0;
+        k1 = DIR == 0 ? sg : 0.0;
+        k2 = DIR == 1 ? sg : 0.0;
+        k3 = DIR == 2 ? sg : 0.0;
+        sigma = fabs(a);
         J = g.uJ;
     } else if (KIND == OCFD_GRID_STRETCHED) {
         const double rx = __ldg(g.rmet[0] + ip), ry = __ldg(g.rmet[1] + jp), rz = __ldg(g.rmet[2] + kp);
-        a1 = DIR == 0 ? ry * rz : 0.0;
-        a2 = DIR == 1 ? rx * rz : 0.0;
-        a3 = DIR == 2 ? rx * ry : 0.0;
+        const double a = DIR == 0 ? ry * rz : DIR == 1 ? rx * rz : rx * ry;
+        const double sg = a < 0.0 ? -1.0 : 1.0;
+        k1 = DIR == 0 ? sg : 0.0;
+        k2 = DIR == 1 ? sg : 0.0;
+        k3 = DIR == 2 ? sg : 0.0;
+        sigma = fabs(a);
         J = (__ldg(g.met[0] + ip) * __ldg(g.met[4] + jp)) * __ldg(g.met[8] + kp);
     } else {
         const double *t = g.atab[DIR] + (long long)kp * g.msk + (long long)jp * g.sy + ip;
-        a1 = __ldg(t);
-        a2 = __ldg(t + g.atab_fs);
-        a3 = __ldg(t + 2 * g.atab_fs);
-        J = __ldg(t + 3 * g.atab_fs);
+        k1 = __ldg(t);
+        k2 = __ldg(t + g.atab_fs);
+        k3 = __ldg(t + 2 * g.atab_fs);
+        sigma = __ldg(t + 3 * g.atab_fs);
+        J = __ldg(t + 4 * g.atab_fs);
     }
 }
 
@@ -173,6 +191,7 @@ ocfd_status launch_prim(ocfd_ctx *c, const double *U);
 ocfd_status launch_sensor(ocfd_ctx *c, const double *U);
 ocfd_status launch_flags(ocfd_ctx *c, unsigned char *flags);
 ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU);
+ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int dir);  // dir = 1 (y) or 2 (z)
 ocfd_status launch_viscous(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage);
 ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage);
 ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);

@@ -1,0 +1,129 @@
+// Device functions shared by the inviscid sweep kernels: the reconstructions of eq. 41 / L286-305 (UD7, WENO7, WENO5),
+// the hybrid interface flag (eq. 42, R-12) and the Steger-Warming split of one point (eq. 19-29).
+#pragma once
+#include "ocfd_internal.cuh"
+
+namespace {
+
+// ------------------------------------------------------------------------------------------ schemes
+// eq. 41 coefficients / 420, in constant memory so that every DFMA takes its coefficient as a constant-bank operand
+__constant__ double c_ud7[7] = {-3.0 / 420.0, 25.0 / 420.0, -101.0 / 420.0, 319.0 / 420.0, 214.0 / 420.0, -38.0 / 420.0, 4.0 / 420.0};
+
+__device__ __forceinline__ double ud7(double a, double b, double c, double d, double e, double f, double g) {
+    // eq. 41, as two fused-multiply-add chains
+    const double lo = fma(c_ud7[2], c, fma(c_ud7[1], b, c_ud7[0] * a));
+    const double hi = fma(c_ud7[6], g, fma(c_ud7[5], f, fma(c_ud7[4], e, c_ud7[3] * d)));
+    return lo + hi;
+}
+
+// WENO7.  Inputs f_{j-3..j+3} in upwind order; one division per reconstruction:
+// sum_k w_k q_k = (sum_k C_k P_k q_k) / (sum_k C_k P_k), P_k = prod_{m != k} (eps + IS_m)^2.
+__device__ __forceinline__ double weno7(double a, double b, double c, double d, double e, double f, double g, double eps) {
+    // undivided differences
+    const double d1a = b - a, d1b = c - b, d1c = d - c, d1d = e - d, d1e = f - e, d1f = g - f;
+    const double d2a = d1b - d1a, d2b = d1c - d1b, d2c = d1d - d1c, d2d = d1e - d1d, d2e = d1f - d1e;
+    const double s30 = d2b - d2a, s31 = d2c - d2b, s32 = d2d - d2c, s33 = d2e - d2d;  // third derivatives
+    // second derivatives of the four cubics at x_j
+    const double s20 = d2b + s30, s21 = d2c, s22 = d2c, s23 = d2d - s33;
+    // first derivatives at x_j
+    const double s10 = (-7.0 * a + 33.0 * b - 69.0 * c + 43.0 * d) * (1.0 / 24.0);
+    const double s11 = (5.0 * b - 27.0 * c + 15.0 * d + 7.0 * e) * (1.0 / 24.0);
+    const double s12 = (-7.0 * c - 15.0 * d + 27.0 * e - 5.0 * f) * (1.0 / 24.0);
+    const double s13 = (-43.0 * d + 69.0 * e - 33.0 * f + 7.0 * g) * (1.0 / 24.0);
+    const double k2 = 13.0 / 12.0, k3 = 1043.0 / 960.0, k13 = 1.0 / 12.0;
+    double i0 = s10 * (s10 + k13 * s30) + k2 * s20 * s20 + k3 * s30 * s30 + eps;
+    double i1 = s11 * (s11 + k13 * s31) + k2 * s21 * s21 + k3 * s31 * s31 + eps;
+    double i2 = s12 * (s12 + k13 * s32) + k2 * s22 * s22 + k3 * s32 * s32 + eps;
+    double i3 = s13 * (s13 + k13 * s33) + k2 * s23 * s23 + k3 * s33 * s33 + eps;
+    i0 *= i0; i1 *= i1; i2 *= i2; i3 *= i3;
+    const double p01 = i0 * i1, p23 = i2 * i3;
+    const double w0 = (1.0 / 35.0) * (i1 * p23), w1 = (12.0 / 35.0) * (i0 * p23);
+    const double w2 = (18.0 / 35.0) * (p01 * i3), w3 = (4.0 / 35.0) * (p01 * i2);
+    const double q0 = (-3.0 * a + 13.0 * b - 23.0 * c + 25.0 * d) * (1.0 / 12.0);
+    const double q1 = (b - 5.0 * c + 13.0 * d + 3.0 * e) * (1.0 / 12.0);
+    const double q2 = (-c + 7.0 * d + 7.0 * e - f) * (1.0 / 12.0);
+    const double q3 = (3.0 * d + 13.0 * e - 5.0 * f + g) * (1.0 / 12.0);
+    return (w0 * q0 + w1 * q1 + w2 * q2 + w3 * q3) / (w0 + w1 + w2 + w3);
+}
+
+// WENO5 (Jiang-Shu), inputs f_{j-2..j+2}
+__device__ __forceinline__ double weno5(double b, double c, double d, double e, double f, double eps) {
+    double t0 = b - 2.0 * c + d, t1 = b - 4.0 * c + 3.0 * d;
+    double i0 = (13.0 / 12.0) * t0 * t0 + 0.25 * t1 * t1 + eps;
+    t0 = c - 2.0 * d + e; t1 = c - e;
+    double i1 = (13.0 / 12.0) * t0 * t0 + 0.25 * t1 * t1 + eps;
+    t0 = d - 2.0 * e + f; t1 = 3.0 * d - 4.0 * e + f;
+    double i2 = (13.0 / 12.0) * t0 * t0 + 0.25 * t1 * t1 + eps;
+    i0 *= i0; i1 *= i1; i2 *= i2;
+    const double w0 = 0.1 * (i1 * i2), w1 = 0.6 * (i0 * i2), w2 = 0.3 * (i0 * i1);
+    const double q0 = (2.0 * b - 7.0 * c + 11.0 * d) * (1.0 / 6.0);
+    const double q1 = (-c + 5.0 * d + 2.0 * e) * (1.0 / 6.0);
+    const double q2 = (2.0 * d + 5.0 * e - f) * (1.0 / 6.0);
+    return (w0 * q0 + w1 * q1 + w2 * q2) / (w0 + w1 + w2);
+}
+
+template <int SCHEME>
+__device__ __forceinline__ double recon(int flag, double a, double b, double c, double d, double e, double f, double g,
+                                        double eps) {
+    if (SCHEME == OCFD_UD7) return ud7(a, b, c, d, e, f, g);
+    if (SCHEME == OCFD_WENO7) return weno7(a, b, c, d, e, f, g, eps);
+    if (SCHEME == OCFD_WENO5) return weno5(b, c, d, e, f, eps);
+    if (flag == 0) return ud7(a, b, c, d, e, f, g);
+    if (flag == 1) return weno7(a, b, c, d, e, f, g, eps);
+    return weno5(b, c, d, e, f, eps);
+}
+
+__device__ __forceinline__ int iface_flag(const GasDesc &gs, double tha, double thb) {
+    double Th = fmax(tha, thb);
+    return Th <= gs.theta1 ? 0 : (Th <= gs.theta2 ? 1 : 2);
+}
+
+// ------------------------------------------------------------------------------------------ Steger-Warming
+// Split fluxes of direction DIR at one point, written to sF[c*cs], c = 0..9 (eq. 19-29 with the
+// readings R-4, R-5, R-7).  k = alpha/|alpha| (unit), sigma = |alpha|, alpha = (d_x,d_y,d_z)/J.
+//
+// With |k| = 1 the bracket of eq. 23-26 collapses: writing A = 2(gamma-1) lam1, S = lam4 + lam5, D = lam5 - lam4,
+//   f1   = h (A + S),                      h = rho / (2 gamma)
+//   f2-4 = u_i f1 + k_i (h c D)
+//   f5   = (q^2/2) f1 + (k.u)(h c D) + (1/2 + (3-gamma)/(2(gamma-1))) c^2 h S
+// (expand (u -+ c k)^2/2 = q^2/2 -+ c k.u + c^2/2), which is 15 instructions per sign instead of 37.
+template <int KIND, int DIR>
+__device__ __forceinline__ void sw_split_store(const GasDesc &gs, double rho, double u, double v, double w, double c,
+                                               double k1, double k2, double k3, double sigma,
+                                               double *__restrict__ sF, int cs) {
+    const double Vn = KIND == OCFD_GRID_CURVILINEAR ? k1 * u + k2 * v + k3 * w
+                                                     : (DIR == 0 ? k1 * u : DIR == 1 ? k2 * v : k3 * w);
+    const double l1 = sigma * Vn, cs_ = c * sigma;
+    const double l4 = l1 - cs_, l5 = l1 + cs_;
+    double l1p, l4p, l5p;
+    if (gs.sw_eps == 0.0) {  // eq. 29
+        l1p = 0.5 * (l1 + fabs(l1)); l4p = 0.5 * (l4 + fabs(l4)); l5p = 0.5 * (l5 + fabs(l5));
+    } else {
+        const double e2 = gs.sw_eps * gs.sw_eps;
+        l1p = 0.5 * (l1 + sqrt(l1 * l1 + e2)); l4p = 0.5 * (l4 + sqrt(l4 * l4 + e2)); l5p = 0.5 * (l5 + sqrt(l5 * l5 + e2));
+    }
+    const double l1m = l1 - l1p, l4m = l4 - l4p, l5m = l5 - l5p;
+    const double h = rho * gs.inv2g;
+    const double hq = 0.5 * (u * u + v * v + w * w);
+    const double hc = h * c, hcc = hc * (c * gs.w1);
+    {
+        const double S = l4p + l5p;
+        const double f1 = h * (gs.tgm1 * l1p + S), D = hc * (l5p - l4p);
+        sF[0] = f1;
+        sF[cs] = KIND == OCFD_GRID_CURVILINEAR || DIR == 0 ? u * f1 + k1 * D : u * f1;
+        sF[2 * cs] = KIND == OCFD_GRID_CURVILINEAR || DIR == 1 ? v * f1 + k2 * D : v * f1;
+        sF[3 * cs] = KIND == OCFD_GRID_CURVILINEAR || DIR == 2 ? w * f1 + k3 * D : w * f1;
+        sF[4 * cs] = hq * f1 + (Vn * D + hcc * S);
+    }
+    {
+        const double S = l4m + l5m;
+        const double f1 = h * (gs.tgm1 * l1m + S), D = hc * (l5m - l4m);
+        sF[5 * cs] = f1;
+        sF[6 * cs] = KIND == OCFD_GRID_CURVILINEAR || DIR == 0 ? u * f1 + k1 * D : u * f1;
+        sF[7 * cs] = KIND == OCFD_GRID_CURVILINEAR || DIR == 1 ? v * f1 + k2 * D : v * f1;
+        sF[8 * cs] = KIND == OCFD_GRID_CURVILINEAR || DIR == 2 ? w * f1 + k3 * D : w * f1;
+        sF[9 * cs] = hq * f1 + (Vn * D + hcc * S);
+    }
+}
+
+}  // namespace
