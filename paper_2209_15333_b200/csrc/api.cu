@@ -144,6 +144,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->inv.ready = false;
     c->inv.U = c->inv.dU = nullptr;
     c->march.ready = false;
+    c->sens_ready = false;
     c->march.U = c->march.dU = nullptr;
     c->visc.ready = false;
     c->visc.Up = c->visc.dUp = nullptr;

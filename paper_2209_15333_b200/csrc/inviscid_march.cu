@@ -26,8 +26,10 @@ constexpr int MR = 4;               // rows per chunk
 constexpr int MNST = 3;             // input stages
 constexpr int MPTS = MAC * MR;      // points per chunk
 constexpr int MNT = 5 * MAC;        // threads: one walker per (pencil, component)
-constexpr int MSTG = 6 * MPTS;      // doubles per input stage: rho, u, v, w, c, theta
-constexpr size_t M_SMEM = sizeof(double) * (size_t)(MNST * MSTG + 10 * MPTS + 2 * 5 * MPTS) + 8 * MNST + 4 * MAC;
+constexpr int MSTG = 10 * MPTS;     // doubles per input stage: rho, u, v, w, c, theta, then k1, k2, k3, sigma (curvilinear)
+constexpr int MNJ = 4;              // slots of the J ring (curvilinear): J of chunk c is used while chunk c+1 is pushed
+constexpr size_t M_SMEM =
+    sizeof(double) * (size_t)(MNST * MSTG + MNJ * MPTS + 10 * MPTS + 2 * 5 * MPTS) + 8 * MNST + 4 * MAC;
 static_assert(MPTS <= MNT && (MPTS * 8) % 128 == 0, "chunk shape");
 
 // J along one pencil of the sweep: at(g, i0, e) = J at padded row i0 + e
@@ -76,10 +78,12 @@ template <int KIND, int SCHEME, int DIR>
 __global__ void __launch_bounds__(MNT, 4)
     k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
                      const __grid_constant__ CUtensorMap tm_prim, const __grid_constant__ CUtensorMap tm_th,
-                     const __grid_constant__ CUtensorMap tm_out) {
+                     const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_met,
+                     const __grid_constant__ CUtensorMap tm_metJ, const int mfull) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double *sIn = reinterpret_cast<double *>(smem_raw);   // [MNST][6][MR][MAC]
-    double *sF = sIn + MNST * MSTG;                       // [10][MR][MAC]: f+ (0..4), f- (5..9) of the current chunk
+    double *sIn = reinterpret_cast<double *>(smem_raw);   // [MNST][10][MR][MAC]
+    double *sJ = sIn + MNST * MSTG;                       // [MNJ][MR][MAC]
+    double *sF = sJ + MNJ * MPTS;                         // [10][MR][MAC]: f+ (0..4), f- (5..9) of the current chunk
     double *sO = sF + 10 * MPTS;                          // [2][5][MR][MAC] output tiles
     uint64_t *bars = reinterpret_cast<uint64_t *>(sO + 2 * 5 * MPTS);
     unsigned char *sFl = reinterpret_cast<unsigned char *>(bars + MNST);   // [MAC][MR] scheme flags pf of the chunk
@@ -96,7 +100,16 @@ __global__ void __launch_bounds__(MNT, 4)
         const int c0 = OCFD_NG + a0;
         const int c1 = DIR == 1 ? MR * c : OCFD_NG + cross;
         const int c2 = DIR == 2 ? MR * c : OCFD_NG + cross;
-        tma::mbar_expect_tx(&bars[s], (SCHEME == OCFD_HYBRID ? 6 : 5) * MPTS * 8);
+        // curvilinear grids: the metric tables k1, k2, k3, sigma and J of the chunk come the same way (mfull = 0: a
+        // z-extruded map swept along z, one row serves the whole chunk)
+        const uint32_t mbytes = KIND == OCFD_GRID_CURVILINEAR ? 5u * (mfull ? MPTS : MAC) * 8u : 0u;
+        tma::mbar_expect_tx(&bars[s], (SCHEME == OCFD_HYBRID ? 6 : 5) * MPTS * 8 + mbytes);
+        if (KIND == OCFD_GRID_CURVILINEAR) {
+            const int m1 = DIR == 1 ? MR * c : OCFD_NG + cross;
+            const int m2 = DIR == 1 ? (g.msk ? OCFD_NG + cross : 0) : (mfull ? MR * c : 0);
+            tma::load4(dst + 6 * MPTS, &tm_met, &bars[s], c0, m1, m2, 0);
+            tma::load4(sJ + (c % MNJ) * MPTS, &tm_metJ, &bars[s], c0, m1, m2, 4);
+        }
         tma::load4(dst, &tm_rho, &bars[s], c0, c1, c2, 0);
         tma::load4(dst + MPTS, &tm_prim, &bars[s], c0, c1, c2, P_U);
         if (SCHEME == OCFD_HYBRID) tma::load4(dst + 5 * MPTS, &tm_th, &bars[s], c0, c1, c2, 0);
@@ -137,18 +150,29 @@ __global__ void __launch_bounds__(MNT, 4)
         double k1 = 0.0, k2 = 0.0, k3 = 0.0, sig = 1.0, Jdead;
         const int rowA = r0 + pr;
         const bool validA = producer && x_ok && rowA < ndp;
-        if (validA)
+        if (KIND != OCFD_GRID_CURVILINEAR && validA)
             met_ksJ<KIND, DIR>(g, ipA, DIR == 1 ? rowA : OCFD_NG + cross, DIR == 2 ? rowA : OCFD_NG + cross, k1, k2, k3, sig,
                                Jdead);
         // ... and J of the four points this walker completes in this chunk (padded rows r0-4 .. r0-1; the first
         // chunk completes nothing that is kept)
         double Jw[MR];
-        {
+        if (KIND != OCFD_GRID_CURVILINEAR) {
             const int i0 = max(r0 - OCFD_NG, 0);
 #pragma unroll
             for (int e = 0; e < MR; ++e) Jw[e] = jrow.at(g, i0, e);
         }
         tma::mbar_wait(&bars[s], (c / MNST) & 1);
+        if (KIND == OCFD_GRID_CURVILINEAR) {
+            // the metric box lands densely: field stride = its own row count x MAC
+            const int mi = mfull ? tid : pa, mfs = mfull ? MPTS : MAC;
+            if (validA) {
+                const double *mp = sU + 6 * MPTS + mi;
+                k1 = mp[0]; k2 = mp[mfs]; k3 = mp[2 * mfs]; sig = mp[3 * mfs];
+            }
+            const double *jp = sJ + ((c + MNJ - 1) % MNJ) * MPTS + wa;   // arrived with chunk c-1 (rows r0-4 .. r0-1)
+#pragma unroll
+            for (int e = 0; e < MR; ++e) Jw[e] = jp[mfull ? e * MAC : 0];
+        }
 
         // ---- phase A: split fluxes of the chunk's points; pf(r) = scheme flag of the interface between rows r-1, r
         if (producer) {
@@ -254,8 +278,9 @@ ocfd_status launch_march(ocfd_ctx *c) {
     dim3 grd((g.nx + MAC - 1) / MAC, ncross, 1);
     OCFD_T0(c, K_INV_X + DIR);
     const MarchMaps &M = c->march;
+    const int mfull = DIR == 1 || g.msk != 0;
     k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.rho[DIR], M.prim[DIR], M.th[DIR],
-                                                                        M.out[DIR]);
+                                                                        M.out[DIR], M.met[DIR], M.metJ[DIR], mfull);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
@@ -285,6 +310,16 @@ bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
         const int by = d == 1 ? MR : 1, bz = d == 2 ? MR : 1;
         const int b1[4] = {MAC, by, bz, 1}, b4[4] = {MAC, by, bz, 4}, bo[4] = {MAC, by, bz, 5};
         if (!M.ready) {
+            if (g.kind == OCFD_GRID_CURVILINEAR) {
+                // the derived metric table of this direction: [5][planes][nyp][nxp], one plane if z-extruded
+                const long long mdim[4] = {g.nxp, g.nyp, g.msk ? g.nzp : 1, 5};
+                const int mz = d == 2 && g.msk ? MR : 1;
+                const int m4[4] = {MAC, by, mz, 4}, m1[4] = {MAC, by, mz, 1};
+                if (!ocfd_tma_encode(&M.met[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m4)) return false;
+                if (!ocfd_tma_encode(&M.metJ[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m1)) return false;
+            } else {   // unused, but the kernel takes the parameters
+                M.met[d] = M.metJ[d] = CUtensorMap();
+            }
             if (!ocfd_tma_encode(&M.prim[d], c->prim, full6, g.sy, g.sz, g.np, b4)) return false;
             if (!ocfd_tma_encode(&M.th[d], c->theta, full1, g.sy, g.sz, g.np, b1)) return false;
         }

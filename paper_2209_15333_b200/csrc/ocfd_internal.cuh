@@ -61,7 +61,7 @@ struct InvMaps {
 struct MarchMaps {
     const double *U, *dU;
     bool ready;
-    CUtensorMap rho[3], prim[3], th[3], out[3];
+    CUtensorMap rho[3], prim[3], th[3], out[3], met[3], metJ[3];
 };
 // ... and of the two viscous passes
 struct ViscMaps {
@@ -88,6 +88,8 @@ struct ocfd_ctx {
     unsigned char *flags;  // [3][np] bytes (debug only)
     InvMaps inv;
     MarchMaps march;
+    CUtensorMap sens_map;   // p with a 1-point x-y halo (shock sensor)
+    bool sens_ready;
     ViscMaps visc;
     long long launches;
     // optional per-launch timing with CUDA events on the launch stream (ocfd_timing)

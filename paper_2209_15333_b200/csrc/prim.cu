@@ -1,5 +1,6 @@
 // Rows a2 (primitives), a3 (shock sensor) and a9 (max wavespeed).
 #include "ocfd_internal.cuh"
+#include "tma.cuh"
 
 namespace {
 
@@ -24,29 +25,74 @@ __global__ void __launch_bounds__(256) k_prim(long long np, GasDesc gs, const do
     }
 }
 
-__device__ __forceinline__ double phi_of(double pm, double p0, double pp) {
-    return fabs(-pm + 2.0 * p0 - pp) / (pm + 2.0 * p0 + pp);  // eq. 42
-}
+// a3: theta = phi_i + phi_j + phi_k at interior points (eq. 42, R-11) and its first ghost layer (R-12).
+// phi_d = |p_- - 2 p_0 + p_+| / (p_- + 2 p_0 + p_+); the three quotients share one division:
+// theta = (n_i d_j d_k + n_j d_i d_k + n_k d_i d_j) / (d_i d_j d_k).
+//
+// 2.5-D marching kernel: a CTA owns an ST x SY tile in x-y and walks along z; every plane of p (with its 1-point x-y
+// halo) is fetched once by a TMA box load into a ring of shared-memory stages that runs ahead of the arithmetic, so
+// p is read once from HBM (8 B/point) and theta written once (8 B/point).
+constexpr int ST = 32, SY = 8, SNT = ST * SY;
+constexpr int SBX = ST + 4, SBY = SY + 2;          // box with halo; 2 wider in x on each side: a box of doubles starts at an even x
+constexpr int S_NST = 6;                           // ring: planes k-1, k, k+1 live, three more in flight
+constexpr int S_STAGE = (SBX * SBY * 8 + 127) / 128 * 128 / 8;   // doubles per stage, 128-byte aligned
+constexpr size_t S_SMEM = sizeof(double) * S_NST * S_STAGE + 8 * S_NST;
 
-// a3: theta = phi_i + phi_j + phi_k at interior points (eq. 42, R-11) and its first ghost layer (R-12)
-__global__ void __launch_bounds__(256) k_sensor(GridDesc g, const double *__restrict__ p, double *__restrict__ theta) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    int j = blockIdx.y * blockDim.y + threadIdx.y;
-    int k = blockIdx.z * blockDim.z + threadIdx.z;
-    if (i >= g.nx || j >= g.ny || k >= g.nz) return;
-    long long id = pidx(g, i + OCFD_NG, j + OCFD_NG, k + OCFD_NG);
-    double p0 = p[id];
-    double th = phi_of(p[id - 1], p0, p[id + 1]);
-    th += phi_of(p[id - g.sy], p0, p[id + g.sy]);
-    th += phi_of(p[id - g.sz], p0, p[id + g.sz]);
-    theta[id] = th;
-    const int c[3] = {i, j, k};
-    const int n[3] = {g.nx, g.ny, g.nz};
-    const long long s[3] = {1, g.sy, g.sz};
+__global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, const __grid_constant__ CUtensorMap tm_p,
+                                                double *__restrict__ theta, int zchunk) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *ring = reinterpret_cast<double *>(smem_raw);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(ring + S_NST * S_STAGE);
+    const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * ST + tx;
+    const int i0 = blockIdx.x * ST, j0 = blockIdx.y * SY;
+    const int i = i0 + tx, j = j0 + ty;
+    const bool own = i < g.nx && j < g.ny;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
+    // plane q of the march = interior plane k0 - 1 + q; stage q % S_NST
+    const int nplanes = k1 - k0 + 2;
+    auto issue = [&](int q) {
+        const int s = q % S_NST;
+        tma::mbar_expect_tx(&bars[s], SBX * SBY * 8);
+        tma::load4(ring + s * S_STAGE, &tm_p, &bars[s], i0 + OCFD_NG - 2, j0 + OCFD_NG - 1, k0 - 1 + q + OCFD_NG, P_P);
+    };
+    if (tid == 0) {
+        for (int s = 0; s < S_NST; ++s) tma::mbar_init(&bars[s], 1);
+        tma::fence_barrier_init();
+        for (int q = 0; q < S_NST && q < nplanes; ++q) issue(q);
+    }
+    __syncthreads();
+    const int ctr = (ty + 1) * SBX + tx + 2;
+    tma::mbar_wait(&bars[0], 0);
+    tma::mbar_wait(&bars[1], 0);
+    double pm = ring[ctr], p0 = ring[S_STAGE + ctr];
+    for (int k = k0; k < k1; ++k) {
+        const int q = k - k0 + 2;   // plane k+1
+        const int s = q % S_NST;
+        tma::mbar_wait(&bars[s], (q / S_NST) & 1);
+        const double pp = ring[s * S_STAGE + ctr];
+        const double *c = ring + ((q - 1) % S_NST) * S_STAGE + ctr;
+        if (own) {
+            const double t0 = p0 + p0;
+            const double ni = fabs(t0 - c[-1] - c[1]), di = t0 + c[-1] + c[1];
+            const double nj = fabs(t0 - c[-SBX] - c[SBX]), dj = t0 + c[-SBX] + c[SBX];
+            const double nk = fabs(t0 - pm - pp), dk = t0 + pm + pp;
+            const double dij = di * dj;
+            const double th = (ni * (dj * dk) + nj * (di * dk) + nk * dij) / (dij * dk);
+            const long long id = pidx(g, i + OCFD_NG, j + OCFD_NG, k + OCFD_NG);
+            theta[id] = th;
+            const int cc[3] = {i, j, k};
+            const int n[3] = {g.nx, g.ny, g.nz};
+            const long long st[3] = {1, g.sy, g.sz};
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        if (c[d] == 0) theta[g.periodic[d] ? id + n[d] * s[d] : id - s[d]] = th;
-        if (c[d] == n[d] - 1) theta[g.periodic[d] ? id - n[d] * s[d] : id + s[d]] = th;
+            for (int d = 0; d < 3; ++d) {
+                if (cc[d] == 0) theta[g.periodic[d] ? id + n[d] * st[d] : id - st[d]] = th;
+                if (cc[d] == n[d] - 1) theta[g.periodic[d] ? id - n[d] * st[d] : id + st[d]] = th;
+            }
+        }
+        pm = p0;
+        p0 = pp;
+        __syncthreads();   // everyone is done with plane k-1: its stage can be refilled
+        if (tid == 0 && q - 2 + S_NST < nplanes) issue(q - 2 + S_NST);
     }
 }
 
@@ -119,9 +165,21 @@ ocfd_status launch_prim(ocfd_ctx *c, const double *U) {
 ocfd_status launch_sensor(ocfd_ctx *c, const double *U) {
     (void)U;
     const GridDesc &g = c->g;
-    dim3 blk(32, 4, 2), grd((g.nx + 31) / 32, (g.ny + 3) / 4, (g.nz + 1) / 2);
+    if (!c->sens_ready) {
+        const long long d6[4] = {g.nxp, g.nyp, g.nzp, P_NF};
+        const int bx[4] = {SBX, SBY, 1, 1};
+        if (!ocfd_tma_encode(&c->sens_map, c->prim, d6, g.sy, g.sz, g.np, bx)) return OCFD_ECUDA;
+        if (cudaFuncSetAttribute(k_sensor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S_SMEM) != cudaSuccess)
+            return OCFD_ECUDA;
+        c->sens_ready = true;
+    }
+    // enough blocks to fill the SMs a few times over, chunks long enough that the two prologue planes stay cheap
+    const long long tiles = (long long)((g.nx + ST - 1) / ST) * ((g.ny + SY - 1) / SY);
+    int zc = g.nz;
+    while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < 148 * 16) zc = (zc + 1) / 2;
+    dim3 blk(ST, SY, 1), grd((g.nx + ST - 1) / ST, (g.ny + SY - 1) / SY, (g.nz + zc - 1) / zc);
     OCFD_T0(c, K_SENSOR);
-    k_sensor<<<grd, blk, 0, c->stream>>>(g, c->prim + (long long)P_P * g.np, c->theta);
+    k_sensor<<<grd, blk, S_SMEM, c->stream>>>(g, c->sens_map, c->theta, zc);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
