@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdio.h>
 
 #include <vector>
 
@@ -198,9 +199,16 @@ ocfd_status launch_viscous(ocfd_ctx *c, double *dU, double *U, double dt, int rk
 ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage);
 ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
 
-#define OCFD_CHECK_LAUNCH(ctx)                                  \
-    do {                                                        \
-        ocfd_t1(ctx);                                           \
-        (ctx)->launches++;                                      \
-        if (cudaGetLastError() != cudaSuccess) return OCFD_ECUDA; \
+// a failed launch is reported on stderr with the CUDA error text (the C ABI only carries OCFD_ECUDA)
+inline bool ocfd_launch_failed(const char *file, int line) {
+    const cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) return false;
+    fprintf(stderr, "libocfd_b200: CUDA error at %s:%d: %s\n", file, line, cudaGetErrorString(e));
+    return true;
+}
+#define OCFD_CHECK_LAUNCH(ctx)                                        \
+    do {                                                              \
+        ocfd_t1(ctx);                                                 \
+        (ctx)->launches++;                                            \
+        if (ocfd_launch_failed(__FILE__, __LINE__)) return OCFD_ECUDA; \
     } while (0)

@@ -88,6 +88,17 @@ __global__ void __launch_bounds__(VNT, 2)
 #pragma unroll
         for (int a = 0; a < 4; ++a) w[a][q + 4] = ring[q * VF_STAGE + a * BYH * BXW + ctr];
     }
+    // whole-tile tests: away from aperiodic faces every point takes the central stencil and no row test is needed
+    const bool xin = g.periodic[0] || (i0 >= 3 && i0 + TX <= g.nx - 3);
+    const bool yin = g.periodic[1] || (j0 >= 3 && j0 + TY <= g.ny - 3);
+    // z-extruded metrics (one plane): fetched once for the whole march
+    const bool hoist = KIND == OCFD_GRID_CURVILINEAR && g.msk == 0;
+    double m[3][3], iJ = 0.0;
+    if (hoist && own) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) Met<KIND>::row(g, d, i + OCFD_NG, j + OCFD_NG, 0, m[d][0], m[d][1], m[d][2]);
+        iJ = 1.0 / Met<KIND>::J(g, i + OCFD_NG, j + OCFD_NG, 0);
+    }
     for (int k = k0; k < k1; ++k) {
         const int kp = k + OCFD_NG;
         const int sn = (k + 3 - k0) % VF_NST;
@@ -103,15 +114,18 @@ __global__ void __launch_bounds__(VNT, 2)
             double gr[4][3];
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
-                gr[a][0] = d1_line(sp + a * BYH * BXW, 1, i, g.nx, g.periodic[0]);
-                gr[a][1] = d1_line(sp + a * BYH * BXW, BXW, j, g.ny, g.periodic[1]);
+                const double *q = sp + a * BYH * BXW;
+                gr[a][0] = xin ? d1c(q[-3], q[-2], q[-1], q[1], q[2], q[3]) : d1_line(q, 1, i, g.nx, 0);
+                gr[a][1] = yin ? d1c(q[-3 * BXW], q[-2 * BXW], q[-BXW], q[BXW], q[2 * BXW], q[3 * BXW])
+                               : d1_line(q, BXW, j, g.ny, 0);
                 gr[a][2] = d1_seven(w[a], k, g.nz, g.periodic[2]);
             }
             const int ip = i + OCFD_NG, jp = j + OCFD_NG;
-            double m[3][3];
+            if (!hoist) {
 #pragma unroll
-            for (int d = 0; d < 3; ++d) Met<KIND>::row(g, d, ip, jp, kp, m[d][0], m[d][1], m[d][2]);
-            const double iJ = 1.0 / Met<KIND>::J(g, ip, jp, kp);
+                for (int d = 0; d < 3; ++d) Met<KIND>::row(g, d, ip, jp, kp, m[d][0], m[d][1], m[d][2]);
+                iJ = 1.0 / Met<KIND>::J(g, ip, jp, kp);
+            }
             double gx[4], gy[4], gz[4];  // Cartesian gradients of T,u,v,w (chain rule)
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
