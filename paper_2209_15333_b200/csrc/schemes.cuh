@@ -16,34 +16,50 @@ __device__ __forceinline__ double ud7(double a, double b, double c, double d, do
     return lo + hi;
 }
 
+// 1/x for x > 0 in the normal range: hardware seed (about 20 bits) and two Newton steps; a quotient num/den formed
+// with it and corrected once by the residual is within a few ulp of the exact one (the bar on the sweeps is 1e-11)
+__device__ __forceinline__ double fast_div_pos(double num, double den) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(den));
+    r = fma(fma(-den, r, 1.0), r, r);
+    r = fma(fma(-den, r, 1.0), r, r);
+    const double q = num * r;
+    return fma(fma(-den, q, num), r, q);
+}
+
 // WENO7.  Inputs f_{j-3..j+3} in upwind order; one division per reconstruction:
-// sum_k w_k q_k = (sum_k C_k P_k q_k) / (sum_k C_k P_k), P_k = prod_{m != k} (eps + IS_m)^2.
+// sum_k w_k q_k = (sum_k P_k C_k q_k) / (sum_k C_k P_k), P_k = prod_{m != k} (eps + IS_m)^2.
+// Everything is written on the undivided differences of the window (the derivatives s1, s2, s3 of the four cubics at
+// x_j and the candidates C_k q_k are short combinations of them), about 100 fp64 instructions per reconstruction.
 __device__ __forceinline__ double weno7(double a, double b, double c, double d, double e, double f, double g, double eps) {
-    // undivided differences
     const double d1a = b - a, d1b = c - b, d1c = d - c, d1d = e - d, d1e = f - e, d1f = g - f;
     const double d2a = d1b - d1a, d2b = d1c - d1b, d2c = d1d - d1c, d2d = d1e - d1d, d2e = d1f - d1e;
     const double s30 = d2b - d2a, s31 = d2c - d2b, s32 = d2d - d2c, s33 = d2e - d2d;  // third derivatives
     // second derivatives of the four cubics at x_j
-    const double s20 = d2b + s30, s21 = d2c, s22 = d2c, s23 = d2d - s33;
-    // first derivatives at x_j
-    const double s10 = (-7.0 * a + 33.0 * b - 69.0 * c + 43.0 * d) * (1.0 / 24.0);
-    const double s11 = (5.0 * b - 27.0 * c + 15.0 * d + 7.0 * e) * (1.0 / 24.0);
-    const double s12 = (-7.0 * c - 15.0 * d + 27.0 * e - 5.0 * f) * (1.0 / 24.0);
-    const double s13 = (-43.0 * d + 69.0 * e - 33.0 * f + 7.0 * g) * (1.0 / 24.0);
+    const double s20 = d2b + s30, s21 = d2c, s23 = d2d - s33;
+    // first derivatives at x_j: (-7a+33b-69c+43d)/24 = d1c + d2b/2 + 7 s30/24, (5b-27c+15d+7e)/24 = (d1c+d1d)/2 - 5 s31/24,
+    // (-7c-15d+27e-5f)/24 = (d1c+d1d)/2 - 5 s32/24, (-43d+69e-33f+7g)/24 = d1d - d2d/2 + 7 s33/24
+    const double mid = 0.5 * (d1c + d1d);
+    const double s10 = fma(7.0 / 24.0, s30, fma(0.5, d2b, d1c));
+    const double s11 = fma(-5.0 / 24.0, s31, mid);
+    const double s12 = fma(-5.0 / 24.0, s32, mid);
+    const double s13 = fma(7.0 / 24.0, s33, fma(-0.5, d2d, d1d));
     const double k2 = 13.0 / 12.0, k3 = 1043.0 / 960.0, k13 = 1.0 / 12.0;
-    double i0 = s10 * (s10 + k13 * s30) + k2 * s20 * s20 + k3 * s30 * s30 + eps;
-    double i1 = s11 * (s11 + k13 * s31) + k2 * s21 * s21 + k3 * s31 * s31 + eps;
-    double i2 = s12 * (s12 + k13 * s32) + k2 * s22 * s22 + k3 * s32 * s32 + eps;
-    double i3 = s13 * (s13 + k13 * s33) + k2 * s23 * s23 + k3 * s33 * s33 + eps;
+    double i0 = fma(s10, fma(k13, s30, s10), fma(k2 * s20, s20, fma(k3 * s30, s30, eps)));
+    double i1 = fma(s11, fma(k13, s31, s11), fma(k2 * s21, s21, fma(k3 * s31, s31, eps)));
+    double i2 = fma(s12, fma(k13, s32, s12), fma(k2 * s21, s21, fma(k3 * s32, s32, eps)));
+    double i3 = fma(s13, fma(k13, s33, s13), fma(k2 * s23, s23, fma(k3 * s33, s33, eps)));
     i0 *= i0; i1 *= i1; i2 *= i2; i3 *= i3;
     const double p01 = i0 * i1, p23 = i2 * i3;
-    const double w0 = (1.0 / 35.0) * (i1 * p23), w1 = (12.0 / 35.0) * (i0 * p23);
-    const double w2 = (18.0 / 35.0) * (p01 * i3), w3 = (4.0 / 35.0) * (p01 * i2);
-    const double q0 = (-3.0 * a + 13.0 * b - 23.0 * c + 25.0 * d) * (1.0 / 12.0);
-    const double q1 = (b - 5.0 * c + 13.0 * d + 3.0 * e) * (1.0 / 12.0);
-    const double q2 = (-c + 7.0 * d + 7.0 * e - f) * (1.0 / 12.0);
-    const double q3 = (3.0 * d + 13.0 * e - 5.0 * f + g) * (1.0 / 12.0);
-    return (w0 * q0 + w1 * q1 + w2 * q2 + w3 * q3) / (w0 + w1 + w2 + w3);
+    const double P0 = i1 * p23, P1 = i0 * p23, P2 = p01 * i3, P3 = p01 * i2;
+    // candidates times their linear weights C = (1, 12, 18, 4)/35
+    const double q0 = fma(25.0 / 420.0, d, fma(-23.0 / 420.0, c, fma(13.0 / 420.0, b, (-3.0 / 420.0) * a)));
+    const double q1 = fma(36.0 / 420.0, e, fma(156.0 / 420.0, d, fma(-60.0 / 420.0, c, (12.0 / 420.0) * b)));
+    const double q2 = fma(-18.0 / 420.0, f, fma(126.0 / 420.0, e, fma(126.0 / 420.0, d, (-18.0 / 420.0) * c)));
+    const double q3 = fma(4.0 / 420.0, g, fma(-20.0 / 420.0, f, fma(52.0 / 420.0, e, (12.0 / 420.0) * d)));
+    const double num = fma(P3, q3, fma(P2, q2, fma(P1, q1, P0 * q0)));
+    const double den = fma(4.0 / 35.0, P3, fma(18.0 / 35.0, P2, fma(12.0 / 35.0, P1, (1.0 / 35.0) * P0)));
+    return fast_div_pos(num, den);
 }
 
 // WENO5 (Jiang-Shu), inputs f_{j-2..j+2}
@@ -59,7 +75,7 @@ __device__ __forceinline__ double weno5(double b, double c, double d, double e, 
     const double q0 = (2.0 * b - 7.0 * c + 11.0 * d) * (1.0 / 6.0);
     const double q1 = (-c + 5.0 * d + 2.0 * e) * (1.0 / 6.0);
     const double q2 = (2.0 * d + 5.0 * e - f) * (1.0 / 6.0);
-    return (w0 * q0 + w1 * q1 + w2 * q2) / (w0 + w1 + w2);
+    return fast_div_pos(w0 * q0 + w1 * q1 + w2 * q2, w0 + w1 + w2);
 }
 
 template <int SCHEME>
