@@ -27,8 +27,8 @@
  *                           quadrature of their integral definition; convexity / ENO property
  *   ora_sw_split            f+ + f- == exact flux of eq. 6; one-sidedness when supersonic;
  *                           eigenvalue signs of the split Jacobians; rotational covariance
- *   ora_d1_line             polynomial exactness of interior and closure rows
- *   viscous terms           manufactured solution differentiated symbolically (sympy), 6th order
+ *   ora_d1_line             polynomial exactness of interior and closure rows, 6th and 8th order
+ *   viscous terms           manufactured solution differentiated symbolically (sympy), 6th / 8th order
  *   ora_rk3_update          y' = lambda y closed form 1 + z + z^2/2 + z^3/6 (eq. 45)
  *   ora_rhs (whole)         freestream, conservation, isentropic-vortex order, Sod vs exact Riemann,
  *                           skewed-grid equivalence, hybrid limits
@@ -60,7 +60,10 @@ typedef struct {
     double T_wall[6];
     const double *wall_vn[6];
     const double *inflow[6];
+    int visc_order;          /* 6 (default; 0 means 6) or 8: order of the central scheme of the viscous terms,
+                                PAPER.md:L313 "two such schemes, of sixth and eighth order" */
 } ora_params;
+static int vorder(const ora_params *P) { return P->visc_order == 8 ? 8 : 6; }
 
 /* ---------------------------------------------------------------- indexing */
 static long SX(const ora_params *P) { (void)P; return 1; }
@@ -229,23 +232,36 @@ static double recon(int scheme, const double f[7], double eps) {
 static double d1_interior(const double *f, long st) {
     return (45.0 * (f[st] - f[-st]) - 9.0 * (f[2 * st] - f[-2 * st]) + (f[3 * st] - f[-3 * st])) / 60.0;
 }
-static double d1_closure(const double *f, long st, int s, int n) {
+/* 8th-order central (the second scheme of PAPER.md:L313; the standard coefficients 4/5, -1/5, 4/105, -1/280 of the
+ * 9-point antisymmetric stencil, pinned by polynomial exactness up to degree 8) */
+static double d1_interior8(const double *f, long st) {
+    return (672.0 * (f[st] - f[-st]) - 168.0 * (f[2 * st] - f[-2 * st]) + 32.0 * (f[3 * st] - f[-3 * st])
+            - 3.0 * (f[4 * st] - f[-4 * st])) / 840.0;
+}
+static double d1_int(const double *f, long st, int order) {
+    return order == 8 ? d1_interior8(f, st) : d1_interior(f, st);
+}
+/* aperiodic axis: "second-order unilateral at the boundary point, second-, fourth- and sixth-order
+ * central at the second, third and fourth boundary points"; the fourth row only exists for the 8th-order scheme
+ * (for the 6th-order scheme the fourth point already takes the interior stencil) */
+static double d1_closure(const double *f, long st, int s, int n, int order) {
     /* f points at element s of the line */
     if (s == 0) return (-3.0 * f[0] + 4.0 * f[st] - f[2 * st]) / 2.0;
     if (s == n - 1) return (3.0 * f[0] - 4.0 * f[-st] + f[-2 * st]) / 2.0;
     if (s == 1 || s == n - 2) return (f[st] - f[-st]) / 2.0;
     if (s == 2 || s == n - 3) return (8.0 * (f[st] - f[-st]) - (f[2 * st] - f[-2 * st])) / 12.0;
-    return d1_interior(f, st);
+    if (order == 8 && (s == 3 || s == n - 4)) return d1_interior(f, st);
+    return d1_int(f, st, order);
 }
 /* derivative of a whole line, for the pins; periodic lines wrap */
-void ora_d1_line(const double *f, int n, int is_periodic, double *out) {
+void ora_d1_line(const double *f, int n, int is_periodic, int order, double *out) {
     for (int s = 0; s < n; ++s) {
         if (is_periodic) {
-            double w[7];
-            for (int m = -3; m <= 3; ++m) w[m + 3] = f[((s + m) % n + n) % n];
-            out[s] = d1_interior(w + 3, 1);
+            double w[9];
+            for (int m = -4; m <= 4; ++m) w[m + 4] = f[((s + m) % n + n) % n];
+            out[s] = d1_int(w + 4, 1, order == 8 ? 8 : 6);
         } else {
-            out[s] = d1_closure(f + s, 1, s, n);
+            out[s] = d1_closure(f + s, 1, s, n, order == 8 ? 8 : 6);
         }
     }
 }
@@ -475,7 +491,7 @@ void ora_viscous_flux_point(const ora_params *P, const double g[4][3], const dou
 static double d1_field(const ora_params *P, const double *f, int d, int i, int j, int k) {
     long id = IDX(P, i, j, k), st = dim_stride(P, d);
     int s = d == 0 ? i : d == 1 ? j : k;
-    return periodic(P, d) ? d1_interior(f + id, st) : d1_closure(f + id, st, s, dim_n(P, d));
+    return periodic(P, d) ? d1_int(f + id, st, vorder(P)) : d1_closure(f + id, st, s, dim_n(P, d), vorder(P));
 }
 /* pass 1 at one interior point: prim arrays pu,pv,pw,pT are padded fields valid on interior+face ghosts */
 static void viscous_flux_at(const ora_params *P, const double *pu, const double *pv, const double *pw,
@@ -534,13 +550,14 @@ void ora_rhs(const ora_params *P, const double *U, double *dU) {
                 for (int d = 0; d < 3; ++d)
                     for (int r = 0; r < 4; ++r) Fv[(4 * d + r) * np + id] = o[d][r];
             }
-    /* periodic axes: wrap the flux of that direction into its 3 nearest ghost layers */
+    /* periodic axes: wrap the flux of that direction into the ghost layers its stencil reaches (3 or 4) */
+    const int H = vorder(P) / 2;
     for (int d = 0; d < 3; ++d) {
         if (!periodic(P, d)) continue;
         int n = dim_n(P, d);
-        for (int k = (d == 2 ? -3 : 0); k < (d == 2 ? P->nz + 3 : P->nz); ++k)
-            for (int j = (d == 1 ? -3 : 0); j < (d == 1 ? P->ny + 3 : P->ny); ++j)
-                for (int i = (d == 0 ? -3 : 0); i < (d == 0 ? P->nx + 3 : P->nx); ++i) {
+        for (int k = (d == 2 ? -H : 0); k < (d == 2 ? P->nz + H : P->nz); ++k)
+            for (int j = (d == 1 ? -H : 0); j < (d == 1 ? P->ny + H : P->ny); ++j)
+                for (int i = (d == 0 ? -H : 0); i < (d == 0 ? P->nx + H : P->nx); ++i) {
                     int c[3] = { i, j, k };
                     if (c[d] >= 0 && c[d] < n) continue;
                     int s[3] = { i, j, k };
@@ -578,16 +595,17 @@ static void fv_dir_at(const ora_params *P, const double *U, int d, int i, int j,
     for (int e = 0; e < 3; ++e) {
         long st = dim_stride(P, e);
         int s = e == 0 ? i : e == 1 ? j : k, n = dim_n(P, e);
-        double line[4][7]; /* u,v,w,T at offsets -3..3 along e (only those the stencil touches) */
-        int lo = -3, hi = 3;
+        double line[4][9]; /* u,v,w,T at offsets -H..H along e (only those the stencil touches) */
+        const int H = vorder(P) / 2;
+        int lo = -H, hi = H;
         if (!periodic(P, e)) { if (s + lo < 0) lo = -s; if (s + hi > n - 1) hi = n - 1 - s; }
-        for (int a = 0; a < 4; ++a) for (int o = 0; o < 7; ++o) line[a][o] = NAN;
+        for (int a = 0; a < 4; ++a) for (int o = 0; o < 9; ++o) line[a][o] = NAN;
         for (int o = lo; o <= hi; ++o) {
             ora_prim q = prim_at(P, U, IDX(P, i, j, k) + o * st);
-            line[0][o + 3] = q.u; line[1][o + 3] = q.v; line[2][o + 3] = q.w; line[3][o + 3] = q.T;
+            line[0][o + 4] = q.u; line[1][o + 4] = q.v; line[2][o + 4] = q.w; line[3][o + 4] = q.T;
         }
         for (int a = 0; a < 4; ++a)
-            g[a][e] = periodic(P, e) ? d1_interior(&line[a][3], 1) : d1_closure(&line[a][3], 1, s, n);
+            g[a][e] = periodic(P, e) ? d1_int(&line[a][4], 1, vorder(P)) : d1_closure(&line[a][4], 1, s, n, vorder(P));
     }
     long mi = MIDX(P, i, j, k);
     for (int q = 0; q < 9; ++q) m[q] = P->met[q][mi];
@@ -627,9 +645,10 @@ void ora_rhs_point(const ora_params *P, const double *U, int i, int j, int k, do
     for (int d = 0; d < 3; ++d) {
         int c[3] = { i, j, k };
         int s0 = c[d], n = dim_n(P, d);
-        double line[4][7];
-        for (int r = 0; r < 4; ++r) for (int o = 0; o < 7; ++o) line[r][o] = NAN;
-        int lo = -3, hi = 3;
+        double line[4][9];
+        for (int r = 0; r < 4; ++r) for (int o = 0; o < 9; ++o) line[r][o] = NAN;
+        const int H = vorder(P) / 2;
+        int lo = -H, hi = H;
         if (!periodic(P, d)) { if (s0 + lo < 0) lo = -s0; if (s0 + hi > n - 1) hi = n - 1 - s0; }
         for (int o = lo; o <= hi; ++o) {
             int s = s0 + o;
@@ -637,10 +656,10 @@ void ora_rhs_point(const ora_params *P, const double *U, int i, int j, int k, do
             c[d] = s;
             double f4[4];
             fv_dir_at(P, U, d, c[0], c[1], c[2], f4);
-            for (int r = 0; r < 4; ++r) line[r][o + 3] = f4[r];
+            for (int r = 0; r < 4; ++r) line[r][o + 4] = f4[r];
         }
         for (int r = 0; r < 4; ++r)
-            dsum[d][r] = periodic(P, d) ? d1_interior(&line[r][3], 1) : d1_closure(&line[r][3], 1, s0, n);
+            dsum[d][r] = periodic(P, d) ? d1_int(&line[r][4], 1, vorder(P)) : d1_closure(&line[r][4], 1, s0, n, vorder(P));
     }
     for (int r = 0; r < 4; ++r) {
         acc[r] = 0.0;

@@ -33,6 +33,7 @@ class OraParams(C.Structure):
         ("T_wall", C.c_double * 6),
         ("wall_vn", _dp * 6),
         ("inflow", _dp * 6),
+        ("visc_order", C.c_int),
     ]
 
 
@@ -102,10 +103,10 @@ def sw_split(gamma, rho, u, v, w, c, alpha, sw_eps=0.0):
     return fp, fm
 
 
-def d1_line(f, periodic):
+def d1_line(f, periodic, order=6):
     f = np.ascontiguousarray(f, dtype=np.float64)
     out = np.zeros_like(f)
-    lib().ora_d1_line(_ptr(f), C.c_int(f.size), C.c_int(1 if periodic else 0), _ptr(out))
+    lib().ora_d1_line(_ptr(f), C.c_int(f.size), C.c_int(1 if periodic else 0), C.c_int(order), _ptr(out))
     return out
 
 
@@ -133,6 +134,7 @@ def params_from_case(case):
     P.gamma, P.Ma, P.Re, P.Pr = case.gamma, case.Ma, case.Re, case.Pr
     P.T_ref, P.T_suth = case.T_ref, case.T_suth
     P.inviscid = 1 if case.inviscid else 0
+    P.visc_order = int(getattr(case, "visc_order", 6))
     P.scheme = SCHEMES[case.scheme]
     P.theta1, P.theta2 = case.theta1, case.theta2
     P.weno_eps, P.sw_eps = case.weno_eps, case.sw_eps

@@ -56,6 +56,61 @@ def test_d1_periodic_wraps(ora):
     assert 50 < e1 / e2 < 80      # 2^6 = 64
 
 
+# ------------------------------------------------------------------ 8th-order scheme
+def test_d1_eighth_order_coefficients_are_the_unique_antisymmetric_nine_point_stencil(ora):
+    """The 9-point antisymmetric stencil exact for x, x^3, x^5, x^7 is unique: solve for it and compare with what the
+    oracle applies to unit impulses (4/5, -1/5, 4/105, -1/280)."""
+    m = np.arange(1, 5, dtype=np.float64)
+    A = np.array([2 * m ** (2 * q + 1) for q in range(4)])      # sum_m c_m (m^p - (-m)^p) = p x^(p-1) at x = 0
+    c = np.linalg.solve(A, np.array([1.0, 0.0, 0.0, 0.0]))
+    assert np.allclose(c, [4 / 5, -1 / 5, 4 / 105, -1 / 280], rtol=1e-12)
+    n = 20
+    for k, ck in enumerate(c, start=1):
+        e = np.zeros(n)
+        e[10 + k] = 1.0
+        assert ora.d1_line(e, periodic=True, order=8)[10] == pytest.approx(ck, rel=1e-14)
+        e[:] = 0.0
+        e[10 - k] = 1.0
+        assert ora.d1_line(e, periodic=True, order=8)[10] == pytest.approx(-ck, rel=1e-14)
+
+
+def test_d1_eighth_order_exactness_and_closure_rows(ora):
+    rng = np.random.default_rng(8)
+    n = 18
+    x = np.arange(n, dtype=np.float64)
+    for deg in range(9):
+        coef = rng.uniform(-1, 1, deg + 1) / 10.0 ** np.arange(deg + 1)
+        d = ora.d1_line(Pl.polyval(x, coef), periodic=False, order=8)
+        ref = Pl.polyval(x, Pl.polyder(coef))
+        assert np.allclose(d[4:n - 4], ref[4:n - 4], atol=1e-10)
+    d = ora.d1_line((x - 9.0) ** 9, periodic=False, order=8)
+    assert abs(d[11] - 9 * (x[11] - 9.0) ** 8) > 1.0          # not exact for degree 9
+    # rows 0..3 and mirrored: one-sided 2nd, central 2nd, 4th, 6th (PAPER.md:L313)
+    for row, deg in {0: 2, 1: 2, 2: 4, 3: 6}.items():
+        for dd in range(deg + 1):
+            f = (x - 3.3) ** dd
+            ref = dd * (x - 3.3) ** max(dd - 1, 0) if dd > 0 else 0 * x
+            d = ora.d1_line(f, periodic=False, order=8)
+            assert d[row] == pytest.approx(ref[row], abs=1e-8), (row, dd)
+            assert d[n - 1 - row] == pytest.approx(ref[n - 1 - row], abs=1e-6 * max(1.0, abs(ref[n - 1 - row]))), (row, dd)
+        f = (x - 3.3) ** (deg + 1)
+        assert abs(ora.d1_line(f, periodic=False, order=8)[row] - (deg + 1) * (x[row] - 3.3) ** deg) > 1e-3, row
+    # rows 0..2 are the same rows as in the 6th-order scheme; the 6th-order scheme has no fourth row
+    f = np.sin(0.7 * x)
+    d6, d8 = ora.d1_line(f, periodic=False, order=6), ora.d1_line(f, periodic=False, order=8)
+    assert np.array_equal(d6[:4], d8[:4]) and np.array_equal(d6[-4:], d8[-4:])
+    assert np.all(d6[4:-4] != d8[4:-4])
+
+
+def test_d1_eighth_order_periodic_convergence(ora):
+    errs = []
+    for n in (16, 32):
+        x = 2 * np.pi * np.arange(n) / n
+        d = ora.d1_line(np.sin(x), periodic=True, order=8) / (2 * np.pi / n)
+        errs.append(np.abs(d - np.cos(x)).max())
+    assert 200 < errs[0] / errs[1] < 300      # 2^8 = 256
+
+
 # ------------------------------------------------------------------ manufactured viscous RHS
 def _manufactured(case, const_T=False):
     """Smooth 2pi-periodic u,v,w,T (rho = 1) and the analytic viscous RHS of rows 2-5, via sympy."""
@@ -79,9 +134,10 @@ def _manufactured(case, const_T=False):
                                        + sp.Rational(1, 3) * sp.diff(div, X[i]) for i in range(3)], "numpy"))
 
 
-def _viscous_error(ora, grid, n, const_T=False):
+def _viscous_error(ora, grid, n, const_T=False, order=6):
     from oracle.oracle import Oracle
     case = W.smooth_periodic(n, n, n, grid=grid, Re=50.0, Ma=0.6)
+    case.visc_order = order
     fn, lap = _manufactured(case, const_T)
     X, Y, Z = case.coords
     u, v, w, T, r1, r2, r3, r4 = [np.broadcast_to(a, X.shape) for a in fn(X, Y, Z)]
@@ -108,6 +164,16 @@ def test_viscous_terms_converge_at_sixth_order_to_the_analytic_rhs(ora, grid):
     e1, e2 = _viscous_error(ora, grid, 24), _viscous_error(ora, grid, 48)
     assert e2 < 1e-4
     assert e1 / e2 > 2.0 ** 5.4, (e1, e2)
+
+
+@pytest.mark.parametrize("grid", ["uniform", "wavy"])
+def test_viscous_terms_eighth_order_scheme_converges_faster(ora, grid):
+    """Same manufactured field with the 8th-order central scheme: two applications of an 8th-order derivative.  On the
+    wavy grid the analytic metrics are exact, so the rate is that of the scheme."""
+    e1, e2 = _viscous_error(ora, grid, 24, order=8), _viscous_error(ora, grid, 48, order=8)
+    assert e2 < 3e-6
+    assert e1 / e2 > 2.0 ** 7.2, (e1, e2)
+    assert e2 < 0.2 * _viscous_error(ora, grid, 48, order=6)
 
 
 def test_viscous_constant_viscosity_special_case(ora):
