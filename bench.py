@@ -26,6 +26,12 @@ from paper_2209_15333_b200 import workloads as W  # noqa: E402
 METRIC = "grid_point_rk3_steps_per_sec"
 UNIT = "grid-point RK3 steps/s"
 
+def _with(case, **kw):
+    for k, v in kw.items():
+        setattr(case, k, v)
+    return case
+
+
 # name -> (generator for the GPU workload, generator for the bounded CPU sample of the same workload, note)
 WORKLOADS = {
     "ramp2048x300x256_hybrid": (lambda: W.ramp(), lambda: W.ramp(nx=512, ny=76, nz=32), "BASELINE configs[4]"),
@@ -36,6 +42,9 @@ WORKLOADS = {
     "tgv32_weno7": (lambda: W.tgv(32), lambda: W.tgv(32), "BASELINE configs[0]"),
     "ramp2048x300x256_weno7": (lambda: W.ramp(scheme="weno7"), lambda: W.ramp(nx=512, ny=76, nz=32, scheme="weno7"),
                                "configs[4] grid with WENO7 everywhere (ALU-bound variant)"),
+    "ramp2048x300x256_hybrid_visc8": (lambda: _with(W.ramp(), visc_order=8),
+                                      lambda: _with(W.ramp(nx=512, ny=76, nz=32), visc_order=8),
+                                      "configs[4] grid with the 8th-order central viscous scheme (SURVEY 8(f) NEXT #3)"),
     "ramp512x76x32_hybrid": (lambda: W.ramp(nx=512, ny=76, nz=32), lambda: W.ramp(nx=512, ny=76, nz=32), "small twin"),
     "ramp1024x152x64_hybrid": (lambda: W.ramp(nx=1024, ny=152, nz=64), lambda: W.ramp(nx=512, ny=76, nz=32),
                                "mid-size twin (ncu captures)"),

@@ -84,6 +84,10 @@ typedef struct {
     void *workspace;         /* device scratch, 256-byte aligned, at least ocfd_workspace_bytes() */
     size_t workspace_bytes;
     void *stream;            /* cudaStream_t to enqueue on (0 = default stream) */
+    /* Order of the central scheme of the viscous terms ("two such schemes, of sixth and eighth
+     * order"): 6 (also 0) or 8.  On aperiodic axes the boundary rows are one-sided 2nd order at the boundary point
+     * and central 2nd / 4th (/ 6th for the 8th-order scheme) at the following points. */
+    int visc_order;
 } ocfd_params;
 
 /* Bytes of device scratch a context with these parameters needs; 0 if the parameters are invalid.  Pure. */

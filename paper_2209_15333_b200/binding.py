@@ -42,6 +42,7 @@ class OcfdParams(C.Structure):
         ("inflow", C.c_void_p * 6),
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
         ("stream", C.c_void_p),
+        ("visc_order", C.c_int),
     ]
 
 
@@ -113,6 +114,7 @@ def params_from_case(case):
     P.gamma, P.Ma, P.Re, P.Pr = case.gamma, case.Ma, case.Re, case.Pr
     P.T_ref, P.T_suth = case.T_ref, case.T_suth
     P.inviscid = 1 if case.inviscid else 0
+    P.visc_order = int(getattr(case, "visc_order", 6))
     P.scheme = SCHEMES[case.scheme]
     P.theta1, P.theta2 = case.theta1, case.theta2
     P.weno_eps, P.sw_eps = case.weno_eps, case.sw_eps

@@ -20,6 +20,7 @@ bool valid_params(const ocfd_params *p) {
     if (!(p->gamma > 1.0) || !(p->Ma > 0.0) || !(p->weno_eps > 0.0) || !(p->sw_eps >= 0.0)) return false;
     if (!p->inviscid && (!(p->Re > 0.0) || !(p->Pr > 0.0) || !(p->T_ref > 0.0) || !(p->T_suth >= 0.0))) return false;
     if (p->scheme < OCFD_UD7 || p->scheme > OCFD_HYBRID) return false;
+    if (p->visc_order != 0 && p->visc_order != 6 && p->visc_order != 8) return false;
     if (p->scheme == OCFD_HYBRID && (isnan(p->theta1) || isnan(p->theta2))) return false;
     switch (p->grid_kind) {
         case OCFD_GRID_UNIFORM:
@@ -98,6 +99,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->p = *p;
     c->stream = (cudaStream_t)p->stream;
     c->nsm = nsm;
+    c->visc_order = p->visc_order == 8 ? 8 : 6;
     GridDesc &g = c->g;
     g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
     g.nxp = p->nx + 8; g.nyp = p->ny + 8; g.nzp = p->nz + 8;

@@ -77,6 +77,7 @@ struct ocfd_ctx {
     GridDesc g;
     GasDesc gas;
     cudaStream_t stream;
+    int visc_order;  // 6 or 8 (ocfd_params.visc_order, 0 -> 6)
     int nsm;         // SM count of the device (persistent kernels launch a multiple of it)
     // workspace carve-up (device pointers)
     double *prim;    // [6][np]: T u v w c p

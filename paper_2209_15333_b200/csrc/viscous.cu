@@ -16,41 +16,71 @@ namespace {
 
 constexpr int TX = 32, TY = 8, VNT = TX * TY;  // own points of a tile = threads
 constexpr int BXW = TX + 8;                    // x extent of a box with x halos (i0-4 .. i0+TX+3)
-constexpr int BYH = TY + 6;                    // y extent of a box with y halos (j0-3 .. j0+TY+2)
+template <int ORDER>
+struct VG {                                    // geometry of the scheme of order ORDER (6 or 8)
+    static constexpr int H = ORDER / 2;        // stencil reach
+    static constexpr int BYH = TY + 2 * H;     // y extent of a box with y halos (j0-H .. j0+TY+H-1)
+    static constexpr int W = 2 * H + 1;        // z window
+};
 
 __device__ __forceinline__ double d1c(double m3, double m2, double m1, double p1, double p2, double p3) {
     return (45.0 * (p1 - m1) - 9.0 * (p2 - m2) + (p3 - m3)) * (1.0 / 60.0);
 }
-// first derivative at position s of a line of n from the seven values v[0..6] = f_{s-3..s+3}; closure rows of an
-// aperiodic axis only touch values inside the line
-__device__ __forceinline__ double d1_seven(const double v[7], int s, int n, int periodic) {
-    if (periodic || (s >= 3 && s <= n - 4)) return d1c(v[0], v[1], v[2], v[4], v[5], v[6]);
-    if (s == 0) return (-3.0 * v[3] + 4.0 * v[4] - v[5]) * 0.5;
-    if (s == n - 1) return (3.0 * v[3] - 4.0 * v[2] + v[1]) * 0.5;
-    if (s == 1 || s == n - 2) return (v[4] - v[2]) * 0.5;
-    return (8.0 * (v[4] - v[2]) - (v[5] - v[1])) * (1.0 / 12.0);  // s == 2 or n-3
+// 8th-order central: 4/5, -1/5, 4/105, -1/280
+__device__ __forceinline__ double d1c8(double m4, double m3, double m2, double m1, double p1, double p2, double p3,
+                                       double p4) {
+    return (672.0 * (p1 - m1) - 168.0 * (p2 - m2) + 32.0 * (p3 - m3) - 3.0 * (p4 - m4)) * (1.0 / 840.0);
 }
-// the same from a shared-memory line (p points at position s, stride st)
+// interior stencil of order ORDER on a line (p points at the position, stride st)
+template <int ORDER>
+__device__ __forceinline__ double d1_int(const double *p, int st) {
+    if (ORDER == 8) return d1c8(p[-4 * st], p[-3 * st], p[-2 * st], p[-st], p[st], p[2 * st], p[3 * st], p[4 * st]);
+    return d1c(p[-3 * st], p[-2 * st], p[-st], p[st], p[2 * st], p[3 * st]);
+}
+// first derivative at position s of a line of n; closure rows of an aperiodic axis (one-sided 2nd order
+// at the boundary point, central 2nd / 4th / 6th order at the 2nd / 3rd / 4th point) only touch values inside the line
+template <int ORDER>
 __device__ __forceinline__ double d1_line(const double *p, int st, int s, int n, int periodic) {
-    if (periodic || (s >= 3 && s <= n - 4)) return d1c(p[-3 * st], p[-2 * st], p[-st], p[st], p[2 * st], p[3 * st]);
+    constexpr int H = ORDER / 2;
+    if (periodic || (s >= H && s <= n - 1 - H)) return d1_int<ORDER>(p, st);
     if (s == 0) return (-3.0 * p[0] + 4.0 * p[st] - p[2 * st]) * 0.5;
     if (s == n - 1) return (3.0 * p[0] - 4.0 * p[-st] + p[-2 * st]) * 0.5;
     if (s == 1 || s == n - 2) return (p[st] - p[-st]) * 0.5;
-    return (8.0 * (p[st] - p[-st]) - (p[2 * st] - p[-2 * st])) * (1.0 / 12.0);
+    if (s == 2 || s == n - 3) return (8.0 * (p[st] - p[-st]) - (p[2 * st] - p[-2 * st])) * (1.0 / 12.0);
+    return d1c(p[-3 * st], p[-2 * st], p[-st], p[st], p[2 * st], p[3 * st]);   // ORDER 8, s == 3 or n-4
+}
+// the same from a register window v[0..2H] = f_{s-H..s+H}
+template <int ORDER>
+__device__ __forceinline__ double d1_win(const double *v, int s, int n, int periodic) {
+    constexpr int H = ORDER / 2;
+    if (periodic || (s >= H && s <= n - 1 - H)) {
+        if (ORDER == 8) return d1c8(v[0], v[1], v[2], v[3], v[5], v[6], v[7], v[8]);
+        return d1c(v[0], v[1], v[2], v[4], v[5], v[6]);
+    }
+    if (s == 0) return (-3.0 * v[H] + 4.0 * v[H + 1] - v[H + 2]) * 0.5;
+    if (s == n - 1) return (3.0 * v[H] - 4.0 * v[H - 1] + v[H - 2]) * 0.5;
+    if (s == 1 || s == n - 2) return (v[H + 1] - v[H - 1]) * 0.5;
+    if (s == 2 || s == n - 3) return (8.0 * (v[H + 1] - v[H - 1]) - (v[H + 2] - v[H - 2])) * (1.0 / 12.0);
+    return d1c(v[H - 3], v[H - 2], v[H - 1], v[H + 1], v[H + 2], v[H + 3]);
 }
 
 // ------------------------------------------------------------------------------------------------ a6
 // Input: primitive fields 0..3 = T,u,v,w (valid on interior + face ghosts).  Output Fv[12][np] at interior points,
 // plus, on periodic axes, the three image planes each direction's flux needs beyond the faces (pass 2 fetches plain
 // boxes and cannot wrap).
-constexpr int VF_NST = 6;                       // ring: planes k..k+3 live, two more in flight
-constexpr int VF_STAGE = 4 * BYH * BXW;         // doubles per stage
-constexpr size_t VF_SMEM = sizeof(double) * VF_NST * VF_STAGE + 8 * VF_NST;
+template <int ORDER>
+struct VF {
+    static constexpr int NST = VG<ORDER>::H + 3;                 // ring: planes k..k+H live, two more in flight
+    static constexpr int STAGE = 4 * VG<ORDER>::BYH * BXW;       // doubles per stage
+    static constexpr size_t SMEM = sizeof(double) * NST * STAGE + 8 * NST;
+    static_assert((STAGE * 8) % 128 == 0, "TMA destinations must stay 128-byte aligned");
+};
 
-template <int KIND>
-__global__ void __launch_bounds__(VNT, 2)
+template <int KIND, int ORDER>
+__global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     k_viscous_flux(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_prim,
                    const double *__restrict__ prim, double *__restrict__ Fv, int zchunk) {
+    constexpr int H = VG<ORDER>::H, BYH = VG<ORDER>::BYH, VF_NST = VF<ORDER>::NST, VF_STAGE = VF<ORDER>::STAGE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + VF_NST * VF_STAGE);
@@ -59,11 +89,11 @@ __global__ void __launch_bounds__(VNT, 2)
     const int i = i0 + tx, j = j0 + ty;
     const bool own = i < g.nx && j < g.ny;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
-    const int last = k1 + 2;  // last plane the window needs
+    const int last = k1 + H - 1;  // last plane the window needs
     auto issue = [&](int plane) {  // plane k (interior index) -> stage (k - k0) % NST
         const int s = (plane - k0) % VF_NST;
         tma::mbar_expect_tx(&bars[s], VF_STAGE * 8);
-        tma::load4(ring + s * VF_STAGE, &tm_prim, &bars[s], i0, j0 + 1, plane + OCFD_NG, 0);
+        tma::load4(ring + s * VF_STAGE, &tm_prim, &bars[s], i0, j0 + OCFD_NG - H, plane + OCFD_NG, 0);
     };
     if (tid == 0) {
         for (int s = 0; s < VF_NST; ++s) tma::mbar_init(&bars[s], 1);
@@ -75,22 +105,22 @@ __global__ void __launch_bounds__(VNT, 2)
     // straight from global memory, everything else through the ring.
     const int ipc = min(i, g.nx - 1) + OCFD_NG, jpc = min(j, g.ny - 1) + OCFD_NG;
     const long long col = (long long)jpc * g.sy + ipc;
-    const int ctr = (ty + 3) * BXW + tx + 4;  // own point inside a staged field
-    double w[4][7];
+    const int ctr = (ty + H) * BXW + tx + 4;  // own point inside a staged field
+    double w[4][2 * H + 1];
 #pragma unroll
     for (int a = 0; a < 4; ++a)
 #pragma unroll
-        for (int q = 0; q < 3; ++q) w[a][q + 1] = __ldg(prim + a * g.np + (long long)(k0 - 3 + q + OCFD_NG) * g.sz + col);
+        for (int q = 0; q < H; ++q) w[a][q + 1] = __ldg(prim + a * g.np + (long long)(k0 - H + q + OCFD_NG) * g.sz + col);
     __syncthreads();  // barriers initialised
 #pragma unroll
-    for (int q = 0; q < 3; ++q) {
+    for (int q = 0; q < H; ++q) {
         tma::mbar_wait(&bars[q], 0);
 #pragma unroll
-        for (int a = 0; a < 4; ++a) w[a][q + 4] = ring[q * VF_STAGE + a * BYH * BXW + ctr];
+        for (int a = 0; a < 4; ++a) w[a][q + H + 1] = ring[q * VF_STAGE + a * BYH * BXW + ctr];
     }
     // whole-tile tests: away from aperiodic faces every point takes the central stencil and no row test is needed
-    const bool xin = g.periodic[0] || (i0 >= 3 && i0 + TX <= g.nx - 3);
-    const bool yin = g.periodic[1] || (j0 >= 3 && j0 + TY <= g.ny - 3);
+    const bool xin = g.periodic[0] || (i0 >= H && i0 + TX <= g.nx - H);
+    const bool yin = g.periodic[1] || (j0 >= H && j0 + TY <= g.ny - H);
     // z-extruded metrics (one plane): fetched once for the whole march
     const bool hoist = KIND == OCFD_GRID_CURVILINEAR && g.msk == 0;
     double m[3][3], iJ = 0.0;
@@ -101,13 +131,13 @@ __global__ void __launch_bounds__(VNT, 2)
     }
     for (int k = k0; k < k1; ++k) {
         const int kp = k + OCFD_NG;
-        const int sn = (k + 3 - k0) % VF_NST;
-        tma::mbar_wait(&bars[sn], ((k + 3 - k0) / VF_NST) & 1);
+        const int sn = (k + H - k0) % VF_NST;
+        tma::mbar_wait(&bars[sn], ((k + H - k0) / VF_NST) & 1);
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
 #pragma unroll
-            for (int q = 0; q < 6; ++q) w[a][q] = w[a][q + 1];
-            w[a][6] = ring[sn * VF_STAGE + a * BYH * BXW + ctr];
+            for (int q = 0; q < 2 * H; ++q) w[a][q] = w[a][q + 1];
+            w[a][2 * H] = ring[sn * VF_STAGE + a * BYH * BXW + ctr];
         }
         if (own) {
             const double *sp = ring + ((k - k0) % VF_NST) * VF_STAGE + ctr;
@@ -115,10 +145,9 @@ __global__ void __launch_bounds__(VNT, 2)
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
                 const double *q = sp + a * BYH * BXW;
-                gr[a][0] = xin ? d1c(q[-3], q[-2], q[-1], q[1], q[2], q[3]) : d1_line(q, 1, i, g.nx, 0);
-                gr[a][1] = yin ? d1c(q[-3 * BXW], q[-2 * BXW], q[-BXW], q[BXW], q[2 * BXW], q[3 * BXW])
-                               : d1_line(q, BXW, j, g.ny, 0);
-                gr[a][2] = d1_seven(w[a], k, g.nz, g.periodic[2]);
+                gr[a][0] = xin ? d1_int<ORDER>(q, 1) : d1_line<ORDER>(q, 1, i, g.nx, 0);
+                gr[a][1] = yin ? d1_int<ORDER>(q, BXW) : d1_line<ORDER>(q, BXW, j, g.ny, 0);
+                gr[a][2] = d1_win<ORDER>(w[a], k, g.nz, g.periodic[2]);
             }
             const int ip = i + OCFD_NG, jp = j + OCFD_NG;
             if (!hoist) {
@@ -133,7 +162,7 @@ __global__ void __launch_bounds__(VNT, 2)
                 gy[a] = m[0][1] * gr[a][0] + m[1][1] * gr[a][1] + m[2][1] * gr[a][2];
                 gz[a] = m[0][2] * gr[a][0] + m[1][2] * gr[a][1] + m[2][2] * gr[a][2];
             }
-            const double T = w[0][3], u = w[1][3], v = w[2][3], ww = w[3][3];
+            const double T = w[0][H], u = w[1][H], v = w[2][H], ww = w[3][H];
             const double mu0 = (1.0 + gs.suth) / (T + gs.suth) * T * sqrt(T);  // eq. 15
             const double mu = mu0 * gs.invRe, kc = mu0 * gs.kfac;              // eq. 14
             const double div = gx[1] + gy[2] + gz[3];
@@ -156,8 +185,8 @@ __global__ void __launch_bounds__(VNT, 2)
                 F[id] = f0; F[g.np + id] = f1; F[2 * g.np + id] = f2; F[3 * g.np + id] = f3;
                 if (g.periodic[d]) {  // images beyond the faces of this direction's own axis
                     long long im = -1;
-                    if (c[d] < 3) im = id + n[d] * st[d];
-                    else if (c[d] >= n[d] - 3) im = id - n[d] * st[d];
+                    if (c[d] < H) im = id + n[d] * st[d];
+                    else if (c[d] >= n[d] - H) im = id - n[d] * st[d];
                     if (im >= 0) { F[im] = f0; F[g.np + im] = f1; F[2 * g.np + im] = f2; F[3 * g.np + im] = f3; }
                 }
             }
@@ -171,19 +200,24 @@ __global__ void __launch_bounds__(VNT, 2)
 // RK: 0 = plain accumulate into dU (ocfd_rhs); 1..3 = also apply RK3 stage RK-1 (eq. 45) to U, dU is not written.
 // One stage holds, for plane k: F with x halos, G with y halos, dU, U, U^n of the tile, and H of plane k+3.
 constexpr int VD_NST = 3;
-constexpr int VD_F = 4 * TY * BXW, VD_G = 4 * BYH * TX, VD_H = 4 * TY * TX, VD_C = 5 * TY * TX;
-constexpr int VD_STAGE = VD_F + VD_G + VD_H + 3 * VD_C;
-constexpr size_t VD_SMEM = sizeof(double) * VD_NST * VD_STAGE + 8 * VD_NST;
-static_assert((VD_F * 8) % 128 == 0 && (VD_G * 8) % 128 == 0 && (VD_H * 8) % 128 == 0 && (VD_C * 8) % 128 == 0 &&
-              (VD_STAGE * 8) % 128 == 0 && (VF_STAGE * 8) % 128 == 0, "TMA destinations must stay 128-byte aligned");
+constexpr int VD_F = 4 * TY * BXW, VD_H = 4 * TY * TX, VD_C = 5 * TY * TX;
+template <int ORDER>
+struct VD {
+    static constexpr int G = 4 * VG<ORDER>::BYH * TX;
+    static constexpr int STAGE = VD_F + G + VD_H + 3 * VD_C;
+    static constexpr size_t SMEM = sizeof(double) * VD_NST * STAGE + 8 * VD_NST;
+    static_assert((VD_F * 8) % 128 == 0 && (G * 8) % 128 == 0 && (VD_H * 8) % 128 == 0 && (VD_C * 8) % 128 == 0 &&
+                  (STAGE * 8) % 128 == 0, "TMA destinations must stay 128-byte aligned");
+};
 
-template <int KIND, int RK>
+template <int KIND, int RK, int ORDER>
 __global__ void __launch_bounds__(VNT, 1)
     k_viscous_div(const GridDesc g, const __grid_constant__ CUtensorMap tm_F, const __grid_constant__ CUtensorMap tm_G,
                   const __grid_constant__ CUtensorMap tm_H, const __grid_constant__ CUtensorMap tm_dU,
                   const __grid_constant__ CUtensorMap tm_U, const __grid_constant__ CUtensorMap tm_Un,
                   const double *__restrict__ Fv, double *__restrict__ dU, double *__restrict__ U,
                   double *__restrict__ Un, double dt, int zchunk) {
+    constexpr int HH = VG<ORDER>::H, BYH = VG<ORDER>::BYH, VD_G = VD<ORDER>::G, VD_STAGE = VD<ORDER>::STAGE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + VD_NST * VD_STAGE);
@@ -200,8 +234,8 @@ __global__ void __launch_bounds__(VNT, 1)
         const int xp = i0 + OCFD_NG, yp = j0 + OCFD_NG, kp = k + OCFD_NG;
         tma::mbar_expect_tx(&bars[s], BYTES);
         tma::load4(b, &tm_F, &bars[s], xp - 4, yp, kp, 0);
-        tma::load4(b + VD_F, &tm_G, &bars[s], xp, yp - 3, kp, 4);
-        tma::load4(b + VD_F + VD_G, &tm_H, &bars[s], xp, yp, kp + 3, 8);
+        tma::load4(b + VD_F, &tm_G, &bars[s], xp, yp - HH, kp, 4);
+        tma::load4(b + VD_F + VD_G, &tm_H, &bars[s], xp, yp, kp + HH, 8);
         tma::load4(b + VD_F + VD_G + VD_H, &tm_dU, &bars[s], xp, yp, kp, 0);
         if (LD_U) tma::load4(b + VD_F + VD_G + VD_H + VD_C, &tm_U, &bars[s], xp, yp, kp, 0);
         if (LD_UN) tma::load4(b + VD_F + VD_G + VD_H + 2 * VD_C, &tm_Un, &bars[s], xp, yp, kp, 0);
@@ -212,15 +246,15 @@ __global__ void __launch_bounds__(VNT, 1)
         for (int q = 0; q < VD_NST; ++q)
             if (k0 + q < k1) issue(k0 + q);
     }
-    // z window of the zeta-direction flux H: planes k-3 .. k+2 from global memory, plane k+3 arrives with stage k
+    // z window of the zeta-direction flux H: planes k-H .. k+H-1 from global memory, plane k+H arrives with stage k
     const int ipc = min(i, g.nx - 1) + OCFD_NG, jpc = min(j, g.ny - 1) + OCFD_NG;
     const long long col = (long long)jpc * g.sy + ipc;
     const double *H = Fv + 8 * g.np;
-    double w[4][7];
+    double w[4][2 * HH + 1];
 #pragma unroll
     for (int r = 0; r < 4; ++r)
 #pragma unroll
-        for (int q = 0; q < 6; ++q) w[r][q + 1] = __ldg(H + r * g.np + (long long)(k0 - 3 + q + OCFD_NG) * g.sz + col);
+        for (int q = 0; q < 2 * HH; ++q) w[r][q + 1] = __ldg(H + r * g.np + (long long)(k0 - HH + q + OCFD_NG) * g.sz + col);
     __syncthreads();  // barriers initialised
     const int ctr = ty * TX + tx;
     for (int k = k0; k < k1; ++k) {
@@ -230,8 +264,8 @@ __global__ void __launch_bounds__(VNT, 1)
 #pragma unroll
         for (int r = 0; r < 4; ++r) {
 #pragma unroll
-            for (int q = 0; q < 6; ++q) w[r][q] = w[r][q + 1];
-            w[r][6] = b[VD_F + VD_G + r * TY * TX + ctr];
+            for (int q = 0; q < 2 * HH; ++q) w[r][q] = w[r][q + 1];
+            w[r][2 * HH] = b[VD_F + VD_G + r * TY * TX + ctr];
         }
         if (own) {
             const int ip = i + OCFD_NG, jp = j + OCFD_NG, kp = k + OCFD_NG;
@@ -242,9 +276,9 @@ __global__ void __launch_bounds__(VNT, 1)
             acc[0] = sdU[ctr];
 #pragma unroll
             for (int r = 0; r < 4; ++r) {
-                double sum = d1_line(b + (r * TY + ty) * BXW + tx + 4, 1, i, g.nx, g.periodic[0]);
-                sum += d1_line(b + VD_F + (r * BYH + ty + 3) * TX + tx, TX, j, g.ny, g.periodic[1]);
-                sum += d1_seven(w[r], k, g.nz, g.periodic[2]);
+                double sum = d1_line<ORDER>(b + (r * TY + ty) * BXW + tx + 4, 1, i, g.nx, g.periodic[0]);
+                sum += d1_line<ORDER>(b + VD_F + (r * BYH + ty + HH) * TX + tx, TX, j, g.ny, g.periodic[1]);
+                sum += d1_win<ORDER>(w[r], k, g.nz, g.periodic[2]);
                 acc[r + 1] = sdU[(r + 1) * TY * TX + ctr] + J * sum;
             }
             if (RK == 0) {
@@ -283,6 +317,7 @@ bool encode_maps(ocfd_ctx *c, const double *dU, const double *U) {
     const GridDesc &g = c->g;
     ViscMaps &M = c->visc;
     const long long d6[4] = {g.nxp, g.nyp, g.nzp, P_NF}, d12[4] = {g.nxp, g.nyp, g.nzp, 12}, d5[4] = {g.nxp, g.nyp, g.nzp, 5};
+    const int BYH = TY + c->visc_order;   // TY + 2 H
     const int bp[4] = {BXW, BYH, 1, 4}, bF[4] = {BXW, TY, 1, 4}, bG[4] = {TX, BYH, 1, 4}, bH[4] = {TX, TY, 1, 4};
     const int bC[4] = {TX, TY, 1, 5};
     if (!M.ready) {
@@ -304,42 +339,44 @@ bool encode_maps(ocfd_ctx *c, const double *dU, const double *U) {
     return true;
 }
 
-template <int KIND, int RK>
+template <int KIND, int RK, int ORDER>
 ocfd_status launch_div(ocfd_ctx *c, dim3 grd, dim3 blk, double *dU, double *U, double dt, int zc) {
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_viscous_div<KIND, RK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VD_SMEM) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_viscous_div<KIND, RK, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)VD<ORDER>::SMEM) != cudaSuccess)
             return OCFD_ECUDA;
         attr_set = true;
     }
     const ViscMaps &M = c->visc;
-    k_viscous_div<KIND, RK><<<grd, blk, VD_SMEM, c->stream>>>(c->g, M.F, M.G, M.H, M.dU, RK ? M.U : M.dU, M.Un, c->Fv, dU, U,
+    k_viscous_div<KIND, RK, ORDER><<<grd, blk, VD<ORDER>::SMEM, c->stream>>>(c->g, M.F, M.G, M.H, M.dU, RK ? M.U : M.dU, M.Un, c->Fv, dU, U,
                                                              c->Un, dt, zc);
     return OCFD_OK;
 }
 
-template <int KIND>
+template <int KIND, int ORDER>
 ocfd_status launch_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
     const GridDesc &g = c->g;
     if (!encode_maps(c, dU, rk_stage >= 0 ? U : nullptr)) return OCFD_ECUDA;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_viscous_flux<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VF_SMEM) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_viscous_flux<KIND, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)VF<ORDER>::SMEM) != cudaSuccess)
             return OCFD_ECUDA;
         attr_set = true;
     }
     const int zc = pick_zchunk(g);
     dim3 blk(TX, TY, 1), grd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zc - 1) / zc);
     OCFD_T0(c, K_VISC_FLUX);
-    k_viscous_flux<KIND><<<grd, blk, VF_SMEM, c->stream>>>(g, c->gas, c->visc.prim, c->prim, c->Fv, zc);
+    k_viscous_flux<KIND, ORDER><<<grd, blk, VF<ORDER>::SMEM, c->stream>>>(g, c->gas, c->visc.prim, c->prim, c->Fv, zc);
     OCFD_CHECK_LAUNCH(c);
     OCFD_T0(c, K_VISC_DIV);
     ocfd_status st;
     switch (rk_stage) {
-        case 0: st = launch_div<KIND, 1>(c, grd, blk, dU, U, dt, zc); break;
-        case 1: st = launch_div<KIND, 2>(c, grd, blk, dU, U, dt, zc); break;
-        case 2: st = launch_div<KIND, 3>(c, grd, blk, dU, U, dt, zc); break;
-        default: st = launch_div<KIND, 0>(c, grd, blk, dU, nullptr, 0.0, zc);
+        case 0: st = launch_div<KIND, 1, ORDER>(c, grd, blk, dU, U, dt, zc); break;
+        case 1: st = launch_div<KIND, 2, ORDER>(c, grd, blk, dU, U, dt, zc); break;
+        case 2: st = launch_div<KIND, 3, ORDER>(c, grd, blk, dU, U, dt, zc); break;
+        default: st = launch_div<KIND, 0, ORDER>(c, grd, blk, dU, nullptr, 0.0, zc);
     }
     if (st != OCFD_OK) return st;
     OCFD_CHECK_LAUNCH(c);
@@ -350,9 +387,16 @@ ocfd_status launch_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_st
 
 // rk_stage < 0: dU += viscous terms.  rk_stage = 0,1,2: the same, then U <- RK3 stage update in the same kernel.
 ocfd_status launch_viscous(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
+    if (c->visc_order == 8) {
+        switch (c->g.kind) {
+            case OCFD_GRID_UNIFORM: return launch_kind<OCFD_GRID_UNIFORM, 8>(c, dU, U, dt, rk_stage);
+            case OCFD_GRID_STRETCHED: return launch_kind<OCFD_GRID_STRETCHED, 8>(c, dU, U, dt, rk_stage);
+            default: return launch_kind<OCFD_GRID_CURVILINEAR, 8>(c, dU, U, dt, rk_stage);
+        }
+    }
     switch (c->g.kind) {
-        case OCFD_GRID_UNIFORM: return launch_kind<OCFD_GRID_UNIFORM>(c, dU, U, dt, rk_stage);
-        case OCFD_GRID_STRETCHED: return launch_kind<OCFD_GRID_STRETCHED>(c, dU, U, dt, rk_stage);
-        default: return launch_kind<OCFD_GRID_CURVILINEAR>(c, dU, U, dt, rk_stage);
+        case OCFD_GRID_UNIFORM: return launch_kind<OCFD_GRID_UNIFORM, 6>(c, dU, U, dt, rk_stage);
+        case OCFD_GRID_STRETCHED: return launch_kind<OCFD_GRID_STRETCHED, 6>(c, dU, U, dt, rk_stage);
+        default: return launch_kind<OCFD_GRID_CURVILINEAR, 6>(c, dU, U, dt, rk_stage);
     }
 }

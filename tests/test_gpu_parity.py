@@ -177,6 +177,33 @@ def test_rhs_parity_with_walls(B, Oracle, which):
     assert err.max() <= TOL_RHS
 
 
+@pytest.mark.parametrize("which", ["uniform", "stretched", "wavy", "plate", "ramp"])
+def test_rhs_parity_eighth_order_viscous_scheme(B, Oracle, which):
+    """visc_order = 8: 9-point central stencils, closure rows 2/2/4/6 on aperiodic axes."""
+    if which == "plate":
+        case = W.flat_plate(nx=72, ny=44, nz=24)
+    elif which == "ramp":
+        case = W.ramp(nx=64, ny=44, nz=24, nmodes=12)
+    else:
+        case = W.smooth_periodic(70, 45, 23, grid=which, scheme="ud7", Re=150.0, seed=5)
+    case.visc_order = 8
+    got, ref, U = run_rhs_both(B, Oracle, case)
+    floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
+    err = rel_linf(got, ref, U, floor)
+    assert err.max() <= TOL_RHS
+    case.visc_order = 6          # and the two schemes really differ
+    ref6 = Oracle(case).rhs(Oracle(case).fill_ghosts(case.U0.copy()))[INT]
+    assert rel_linf(ref, ref6, U, floor).max() > 1e-9
+
+
+def test_ten_steps_eighth_order_viscous_scheme(B, Oracle):
+    case = W.tgv(24, nsteps=10)
+    case.visc_order = 8
+    err, _, _ = step_both(B, Oracle, case, 10, check_every=5)
+    print("TGV 24^3, 8th-order viscous scheme, 10 steps: rel Linf", err)
+    assert err <= TOL_100
+
+
 def step_both(B, Oracle, case, nsteps, check_every=None):
     o = Oracle(case)
     U = o.fill_ghosts(case.U0.copy())
