@@ -62,6 +62,8 @@ typedef struct {
     const double *inflow[6];
     int visc_order;          /* 6 (default; 0 means 6) or 8: order of the central scheme of the viscous terms,
                                 PAPER.md:L313 "two such schemes, of sixth and eighth order" */
+    int bc_closure;          /* 0: ghost cells feed the full stencils (north_star; DESIGN R-14);
+                                1: the paper's boundary scheme, PAPER.md:L307-309 (DESIGN R-20, R-21) */
 } ora_params;
 static int vorder(const ora_params *P) { return P->visc_order == 8 ? 8 : 6; }
 
@@ -408,15 +410,60 @@ static void split_at(const ora_params *P, const double *U, int d, int i, int j, 
     double a1 = P->met[3 * d][mi] / J, a2 = P->met[3 * d + 1][mi] / J, a3 = P->met[3 * d + 2][mi] / J; /* PAPER.md:L167 */
     ora_sw_split(P->gamma, P->sw_eps, q.rho, q.u, q.v, q.w, q.c, a1, a2, a3, fp, fm);
 }
+/* Paper's boundary scheme (PAPER.md:L307-309): "uses the fifth-order WENO scheme to calculate the numerical flux near
+ * the boundary.  When a subtemplate of the WENO scheme uses grid points outside the boundary, the weight of the
+ * subtemplate is forced to 0".  f[0..4] is the upwind-oriented WENO5 window, keep bit k set = candidate k lies inside
+ * the domain.  Candidates that are shielded are not evaluated at all (no value outside the domain is read).  If every
+ * candidate is shielded (the interface on the boundary itself, for the flux whose upwind side is outside) the value
+ * of the boundary node `nearest` is taken (DESIGN R-21; the paper is silent). */
+double ora_weno5_masked(const double f[5], double eps, int keep, double nearest) {
+    static const double C[3] = { 0.1, 0.6, 0.3 };
+    double q[3] = { 0, 0, 0 }, al[3] = { 0, 0, 0 }, sum = 0.0, a, b, IS;
+    if ((keep & 7) == 0) return nearest;
+    if (keep & 1) {
+        q[0] = (2.0 * f[0] - 7.0 * f[1] + 11.0 * f[2]) / 6.0;
+        a = f[0] - 2.0 * f[1] + f[2]; b = f[0] - 4.0 * f[1] + 3.0 * f[2];
+        IS = 13.0 / 12.0 * a * a + 0.25 * b * b;
+        al[0] = C[0] / ((eps + IS) * (eps + IS));
+    }
+    if (keep & 2) {
+        q[1] = (-f[1] + 5.0 * f[2] + 2.0 * f[3]) / 6.0;
+        a = f[1] - 2.0 * f[2] + f[3]; b = f[1] - f[3];
+        IS = 13.0 / 12.0 * a * a + 0.25 * b * b;
+        al[1] = C[1] / ((eps + IS) * (eps + IS));
+    }
+    if (keep & 4) {
+        q[2] = (2.0 * f[2] + 5.0 * f[3] - f[4]) / 6.0;
+        a = f[2] - 2.0 * f[3] + f[4]; b = 3.0 * f[2] - 4.0 * f[3] + f[4];
+        IS = 13.0 / 12.0 * a * a + 0.25 * b * b;
+        al[2] = C[2] / ((eps + IS) * (eps + IS));
+    }
+    sum = al[0] + al[1] + al[2];
+    return (al[0] / sum) * q[0] + (al[1] / sum) * q[1] + (al[2] / sum) * q[2];
+}
+static int inside3(int a, int n) { return a >= 0 && a + 2 <= n - 1; } /* points a, a+1, a+2 all in [0, n-1] */
 /* numerical flux h_{s+1/2}[5] along direction d, from the split fluxes of the 8 points s-3..s+4
- * (fp, fm are [8][5], row r = point s-3+r). f+ uses s-3..s+3; f- uses the mirror s+4..s-2. */
-static void iface_flux(int scheme, double eps, const double fp[8][5], const double fm[8][5], double h[5]) {
+ * (fp, fm are [8][5], row r = point s-3+r). f+ uses s-3..s+3; f- uses the mirror s+4..s-2.
+ * closure != 0 (aperiodic axis of n points with the paper's boundary scheme, DESIGN R-20): a flux whose 7-point
+ * stencil reaches outside [0, n-1] is replaced by the shielded WENO5 above, separately for f+ and f-. */
+static void iface_flux(int scheme, double eps, const double fp[8][5], const double fm[8][5], double h[5],
+                       int closure, int s, int n) {
+    const int near_p = closure && (s - 3 < 0 || s + 3 > n - 1);
+    const int near_m = closure && (s - 2 < 0 || s + 4 > n - 1);
+    /* f+ candidates {s-2,s-1,s}, {s-1,s,s+1}, {s,s+1,s+2}; f- (mirrored) {s+3,s+2,s+1}, {s+2,s+1,s}, {s+1,s,s-1} */
+    const int keep_p = inside3(s - 2, n) | inside3(s - 1, n) << 1 | inside3(s, n) << 2;
+    const int keep_m = inside3(s + 1, n) | inside3(s, n) << 1 | inside3(s - 1, n) << 2;
+    const int np_ = s < 0 ? 0 : s > n - 1 ? n - 1 : s;             /* boundary node nearest to the upwind side of f+ */
+    const int nm_ = s + 1 < 0 ? 0 : s + 1 > n - 1 ? n - 1 : s + 1; /* ... of f- */
     for (int m = 0; m < 5; ++m) {
         double a[7], b[7];
         for (int r = 0; r < 7; ++r) { a[r] = fp[r][m]; b[r] = fm[7 - r][m]; }
-        h[m] = recon(scheme, a, eps) + recon(scheme, b, eps);
+        const double hp = near_p ? ora_weno5_masked(a + 1, eps, keep_p, fp[np_ - (s - 3)][m]) : recon(scheme, a, eps);
+        const double hm = near_m ? ora_weno5_masked(b + 1, eps, keep_m, fm[nm_ - (s - 3)][m]) : recon(scheme, b, eps);
+        h[m] = hp + hm;
     }
 }
+static int closure_on(const ora_params *P, int d) { return P->bc_closure && !periodic(P, d); }
 /* dU -= J (h_{s+1/2} - h_{s-1/2}) over all interior points, direction d  (A.1, A.6) */
 static void inviscid_dir(const ora_params *P, const double *U, const double *theta, int d, double *dU) {
     long np = NP(P);
@@ -441,7 +488,8 @@ static void inviscid_dir(const ora_params *P, const double *U, const double *the
                     c[d] = s;
                     long id = IDX(P, c[0], c[1], c[2]);
                     int sch = P->scheme == ORA_HYBRID ? iface_scheme(P, theta[id], theta[id + dim_stride(P, d)]) : P->scheme;
-                    iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + (s - 3 + NG)), (const double(*)[5])(fm + (s - 3 + NG)), h[s + 1]);
+                    iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + (s - 3 + NG)), (const double(*)[5])(fm + (s - 3 + NG)), h[s + 1],
+                               closure_on(P, d), s, n);
                 }
                 for (int s = 0; s < n; ++s) {
                     c[d] = s;
@@ -632,7 +680,8 @@ void ora_rhs_point(const ora_params *P, const double *U, int i, int j, int k, do
                 a[d] = s0 - 1 + e; b[d] = s0 + e;
                 sch = iface_scheme(P, theta_for(P, U, d, a[0], a[1], a[2]), theta_for(P, U, d, b[0], b[1], b[2]));
             }
-            iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + e), (const double(*)[5])(fm + e), h[e]);
+            iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + e), (const double(*)[5])(fm + e), h[e],
+                       closure_on(P, d), s0 - 1 + e, dim_n(P, d));
         }
         for (int m = 0; m < 5; ++m) out[m] -= J * (h[1][m] - h[0][m]);
     }

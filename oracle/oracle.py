@@ -34,6 +34,7 @@ class OraParams(C.Structure):
         ("wall_vn", _dp * 6),
         ("inflow", _dp * 6),
         ("visc_order", C.c_int),
+        ("bc_closure", C.c_int),
     ]
 
 
@@ -88,6 +89,15 @@ def weno5(f, eps=1e-6):
     return lib().ora_weno5(_ptr(f), C.c_double(eps))
 
 
+def weno5_masked(f, keep, nearest, eps=1e-6):
+    """Shielded WENO5 of the paper's boundary scheme; bit k of `keep` = candidate k is inside."""
+    f = np.ascontiguousarray(f, dtype=np.float64)
+    assert f.size == 5
+    L = lib()
+    L.ora_weno5_masked.restype = C.c_double
+    return float(L.ora_weno5_masked(_ptr(f), C.c_double(eps), C.c_int(keep), C.c_double(nearest)))
+
+
 def weno5_parts(f, eps=1e-6):
     f = np.ascontiguousarray(f, dtype=np.float64)
     q, IS, om = np.zeros(3), np.zeros(3), np.zeros(3)
@@ -135,6 +145,7 @@ def params_from_case(case):
     P.T_ref, P.T_suth = case.T_ref, case.T_suth
     P.inviscid = 1 if case.inviscid else 0
     P.visc_order = int(getattr(case, "visc_order", 6))
+    P.bc_closure = int(getattr(case, "bc_closure", 0))
     P.scheme = SCHEMES[case.scheme]
     P.theta1, P.theta2 = case.theta1, case.theta2
     P.weno_eps, P.sw_eps = case.weno_eps, case.sw_eps
