@@ -45,6 +45,9 @@ WORKLOADS = {
     "ramp2048x300x256_hybrid_visc8": (lambda: _with(W.ramp(), visc_order=8),
                                       lambda: _with(W.ramp(nx=512, ny=76, nz=32), visc_order=8),
                                       "configs[4] grid with the 8th-order central viscous scheme (SURVEY 8(f) NEXT #3)"),
+    "ramp2048x300x256_hybrid_closure": (lambda: _with(W.ramp(), bc_closure=1),
+                                        lambda: _with(W.ramp(nx=512, ny=76, nz=32), bc_closure=1),
+                                        "configs[4] with the paper's inviscid boundary scheme (SURVEY 8(f) NEXT #1)"),
     "ramp512x76x32_hybrid": (lambda: W.ramp(nx=512, ny=76, nz=32), lambda: W.ramp(nx=512, ny=76, nz=32), "small twin"),
     "ramp1024x152x64_hybrid": (lambda: W.ramp(nx=1024, ny=152, nz=64), lambda: W.ramp(nx=512, ny=76, nz=32),
                                "mid-size twin (ncu captures)"),

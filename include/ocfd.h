@@ -88,6 +88,13 @@ typedef struct {
      * order"): 6 (also 0) or 8.  On aperiodic axes the boundary rows are one-sided 2nd order at the boundary point
      * and central 2nd / 4th (/ 6th for the 8th-order scheme) at the following points. */
     int visc_order;
+    /* Inviscid boundary scheme on aperiodic axes.  0: the ghost cells written by ocfd_fill_ghosts feed the full
+     * stencils (default).  1: the paper's scheme: a flux whose 7-point stencil reaches outside
+     * the domain is computed by WENO5 with the candidate sub-stencils that contain an outside point shielded
+     * (weight 0, the others renormalised); no value outside the domain is read by the sweeps.  If all three
+     * candidates are shielded (the boundary interface itself, for the wave that enters) the boundary node's split
+     * flux is taken (DESIGN R-21). */
+    int bc_closure;
 } ocfd_params;
 
 /* Bytes of device scratch a context with these parameters needs; 0 if the parameters are invalid.  Pure. */

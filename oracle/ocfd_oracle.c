@@ -32,6 +32,8 @@
  *   ora_rk3_update          y' = lambda y closed form 1 + z + z^2/2 + z^3/6 (eq. 45)
  *   ora_rhs (whole)         freestream, conservation, isentropic-vortex order, Sod vs exact Riemann,
  *                           skewed-grid equivalence, hybrid limits
+ *   ora_weno5_masked        (paper boundary scheme, bc_closure) candidate exactness, renormalised weights, no
+ *                           out-of-domain reads; the all-shielded value (DESIGN R-21) is PARITY UNPINNED
  *   ora_max_wavespeed       uniform-flow closed form; brute force
  *   ora_fill_ghosts         BC invariants
  * Unpinned (no data in the container): agreement with the authors' own program output.

@@ -43,6 +43,7 @@ class OcfdParams(C.Structure):
         ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
         ("stream", C.c_void_p),
         ("visc_order", C.c_int),
+        ("bc_closure", C.c_int),
     ]
 
 
@@ -115,6 +116,7 @@ def params_from_case(case):
     P.T_ref, P.T_suth = case.T_ref, case.T_suth
     P.inviscid = 1 if case.inviscid else 0
     P.visc_order = int(getattr(case, "visc_order", 6))
+    P.bc_closure = int(getattr(case, "bc_closure", 0))
     P.scheme = SCHEMES[case.scheme]
     P.theta1, P.theta2 = case.theta1, case.theta2
     P.weno_eps, P.sw_eps = case.weno_eps, case.sw_eps

@@ -21,6 +21,7 @@ bool valid_params(const ocfd_params *p) {
     if (!p->inviscid && (!(p->Re > 0.0) || !(p->Pr > 0.0) || !(p->T_ref > 0.0) || !(p->T_suth >= 0.0))) return false;
     if (p->scheme < OCFD_UD7 || p->scheme > OCFD_HYBRID) return false;
     if (p->visc_order != 0 && p->visc_order != 6 && p->visc_order != 8) return false;
+    if (p->bc_closure != 0 && p->bc_closure != 1) return false;
     if (p->scheme == OCFD_HYBRID && (isnan(p->theta1) || isnan(p->theta2))) return false;
     switch (p->grid_kind) {
         case OCFD_GRID_UNIFORM:
@@ -113,6 +114,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
         g.uJ = (g.ux * g.uy) * g.uz;
     }
     for (int d = 0; d < 3; ++d) g.periodic[d] = p->bc[2 * d] == OCFD_BC_PERIODIC;
+    for (int d = 0; d < 3; ++d) g.closure[d] = p->bc_closure && !g.periodic[d];
     GasDesc &s = c->gas;
     s.gamma = p->gamma; s.gm1 = p->gamma - 1.0; s.Ma = p->Ma; s.gM2 = p->gamma * p->Ma * p->Ma; s.invMa = 1.0 / p->Ma;
     s.inv2g = 1.0 / (2.0 * p->gamma);

@@ -186,7 +186,10 @@ __global__ void __launch_bounds__(INV_NT, 3)
 #pragma unroll
                 for (int e = 0; e < 5; ++e) mask |= sFl[(seg * 5 + e) * AC + a];
             }
-            const bool smooth = SCHEME == OCFD_UD7 || (SCHEME == OCFD_HYBRID && mask == 0u);
+            // the paper's boundary scheme (ocfd_params.bc_closure): segments with an interface s = o0-1+q within reach of
+            // a boundary (s <= 2 or s >= nd-4) take the general loop, which tests every interface
+            const bool near_bnd = g.closure[DIR] && (o0 - 1 + q0 <= 2 || o0 - 1 + qend - 1 >= nd - 4);
+            const bool smooth = !near_bnd && (SCHEME == OCFD_UD7 || (SCHEME == OCFD_HYBRID && mask == 0u));
             if (smooth) {
                 // every interface of the segment takes the linear scheme: fully unrolled, the windows slide by
                 // renaming (the last segment runs past NIF: its extra loads stay inside the shared-memory
@@ -217,8 +220,12 @@ __global__ void __launch_bounds__(INV_NT, 3)
                     const int flag = SCHEME == OCFD_HYBRID ? (int)((mask >> (2 * (q - q0))) & 3u) : 0;
                     double h = 0.0;
                     if (q < qlive) {
-                        h = recon<SCHEME>(flag, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6], gs.weno_eps) +
-                            recon<SCHEME>(flag, wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
+                        if (near_bnd)
+                            h = recon_pair_closure<SCHEME>(flag, o0 - 1 + q, nd, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6],
+                                                           wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
+                        else
+                            h = recon<SCHEME>(flag, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6], gs.weno_eps) +
+                                recon<SCHEME>(flag, wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
                     }
                     sH[(m * NIF + q) * ACP + a] = h;
                 }

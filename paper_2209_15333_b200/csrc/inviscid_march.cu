@@ -212,6 +212,10 @@ __global__ void __launch_bounds__(MNT, 4)
             pprev = pc;
             fast = cur == 0;
         }
+        // the paper's boundary scheme (ocfd_params.bc_closure): the chunks whose interfaces s = r0-8 .. r0-5 come within
+        // reach of a boundary (s <= 2 or s >= nd-4) take the out-of-line path, which tests every interface
+        const bool near_bnd = g.closure[DIR] && (r0 - 2 * OCFD_NG <= 2 || r0 + MR - 1 - 2 * OCFD_NG >= nd - 4);
+        if (near_bnd) fast = false;
         double nP[MR], nM[MR];   // the chunk's new rows (loaded up front, entered into the rings one by one)
 #pragma unroll
         for (int e = 0; e < MR; ++e) {
@@ -238,10 +242,16 @@ __global__ void __launch_bounds__(MNT, 4)
                 Wp[k & 7] = nP[e];
                 Wm[k & 7] = nM[e];
                 const int flag = SCHEME == OCFD_HYBRID ? (int)((cur >> (2 * e)) & 3u) : 0;
-                const double h = recon_pair<SCHEME>(flag, Wp[(k + 1) & 7], Wp[(k + 2) & 7], Wp[(k + 3) & 7], Wp[(k + 4) & 7],
-                                                    Wp[(k + 5) & 7], Wp[(k + 6) & 7], Wp[(k + 7) & 7], Wm[k & 7],
-                                                    Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
-                                                    Wm[(k + 3) & 7], Wm[(k + 2) & 7], gs.weno_eps);
+                const double h =
+                    near_bnd ? recon_pair_closure<SCHEME>(flag, r0 + e - 2 * OCFD_NG, nd, Wp[(k + 1) & 7], Wp[(k + 2) & 7],
+                                                          Wp[(k + 3) & 7], Wp[(k + 4) & 7], Wp[(k + 5) & 7], Wp[(k + 6) & 7],
+                                                          Wp[(k + 7) & 7], Wm[k & 7], Wm[(k + 7) & 7], Wm[(k + 6) & 7],
+                                                          Wm[(k + 5) & 7], Wm[(k + 4) & 7], Wm[(k + 3) & 7], Wm[(k + 2) & 7],
+                                                          gs.weno_eps)
+                             : recon_pair<SCHEME>(flag, Wp[(k + 1) & 7], Wp[(k + 2) & 7], Wp[(k + 3) & 7], Wp[(k + 4) & 7],
+                                                  Wp[(k + 5) & 7], Wp[(k + 6) & 7], Wp[(k + 7) & 7], Wm[k & 7],
+                                                  Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
+                                                  Wm[(k + 3) & 7], Wm[(k + 2) & 7], gs.weno_eps);
                 so[e * MAC] = -Jw[e] * (h - hprev);
                 hprev = h;
             }

@@ -23,6 +23,7 @@ struct GridDesc {
     double ux, uy, uz;     // uniform: 1/dx, 1/dy, 1/dz
     double uJ;             // uniform: J
     int periodic[3];
+    int closure[3];        // 1: the paper's shielded-WENO5 boundary scheme on this (aperiodic) axis (ocfd_params.bc_closure)
     // derived metric data built once at init (launch_metric_tables), so that no kernel divides by J per point:
     //   curvilinear: atab[d] = [5][planes][nyp][nxp] fields (k1, k2, k3, sigma, J) with alpha = (d_x, d_y, d_z)/J,
     //                sigma = |alpha|, k = alpha/sigma; k-plane stride msk (0 if extruded)

@@ -78,6 +78,33 @@ __device__ __forceinline__ double weno5(double b, double c, double d, double e, 
     return fast_div_pos(w0 * q0 + w1 * q1 + w2 * q2, w0 + w1 + w2);
 }
 
+// WENO5 with shielded candidates (the paper's boundary scheme; DESIGN R-20): bit k of `keep` set =
+// candidate k lies inside the domain; the others get weight 0 and are not evaluated.  keep == 0: `nearest` (R-21).
+__device__ __forceinline__ double weno5_masked(double b, double c, double d, double e, double f, double eps, int keep,
+                                               double nearest) {
+    if ((keep & 7) == 0) return nearest;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, q0 = 0.0, q1 = 0.0, q2 = 0.0;
+    if (keep & 1) {
+        const double t0 = b - 2.0 * c + d, t1 = b - 4.0 * c + 3.0 * d;
+        const double is = (13.0 / 12.0) * t0 * t0 + 0.25 * t1 * t1 + eps;
+        a0 = 0.1 / (is * is);
+        q0 = (2.0 * b - 7.0 * c + 11.0 * d) * (1.0 / 6.0);
+    }
+    if (keep & 2) {
+        const double t0 = c - 2.0 * d + e, t1 = c - e;
+        const double is = (13.0 / 12.0) * t0 * t0 + 0.25 * t1 * t1 + eps;
+        a1 = 0.6 / (is * is);
+        q1 = (-c + 5.0 * d + 2.0 * e) * (1.0 / 6.0);
+    }
+    if (keep & 4) {
+        const double t0 = d - 2.0 * e + f, t1 = 3.0 * d - 4.0 * e + f;
+        const double is = (13.0 / 12.0) * t0 * t0 + 0.25 * t1 * t1 + eps;
+        a2 = 0.3 / (is * is);
+        q2 = (2.0 * d + 5.0 * e - f) * (1.0 / 6.0);
+    }
+    return (a0 * q0 + a1 * q1 + a2 * q2) / (a0 + a1 + a2);
+}
+
 template <int SCHEME>
 __device__ __forceinline__ double recon(int flag, double a, double b, double c, double d, double e, double f, double g,
                                         double eps) {
@@ -92,6 +119,25 @@ __device__ __forceinline__ double recon(int flag, double a, double b, double c, 
 __device__ __forceinline__ int iface_flag(const GasDesc &gs, double tha, double thb) {
     double Th = fmax(tha, thb);
     return Th <= gs.theta1 ? 0 : (Th <= gs.theta2 ? 1 : 2);
+}
+
+// h_{s+1/2} of an interface near an aperiodic boundary under the paper's boundary scheme.  s = interior index of the
+// interface (s + 1/2), n = points of the axis; p0..p6 = f+ of points s-3..s+3, m0..m6 = f- of points s+4..s-2.  A flux
+// whose 7-point stencil stays inside [0, n-1] takes the regular scheme `flag`.  Out of line: it runs on the few
+// interfaces next to a boundary only.
+__device__ __forceinline__ int inside3(int a, int n) { return a >= 0 && a + 2 <= n - 1; }
+template <int SCHEME>
+__device__ __noinline__ double recon_pair_closure(int flag, int s, int n, double p0, double p1, double p2, double p3,
+                                                  double p4, double p5, double p6, double m0, double m1, double m2,
+                                                  double m3, double m4, double m5, double m6, double eps) {
+    const bool near_p = s - 3 < 0 || s + 3 > n - 1, near_m = s - 2 < 0 || s + 4 > n - 1;
+    // f+ candidates {s-2,s-1,s}, {s-1,s,s+1}, {s,s+1,s+2}; f- (mirrored) {s+3,s+2,s+1}, {s+2,s+1,s}, {s+1,s,s-1}
+    const int keep_p = inside3(s - 2, n) | inside3(s - 1, n) << 1 | inside3(s, n) << 2;
+    const int keep_m = inside3(s + 1, n) | inside3(s, n) << 1 | inside3(s - 1, n) << 2;
+    // all shielded only at s = -1 (f+: nearest node 0 = p4) and s = n-1 (f-: nearest node n-1 = m4)
+    const double hp = near_p ? weno5_masked(p1, p2, p3, p4, p5, eps, keep_p, p4) : recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps);
+    const double hm = near_m ? weno5_masked(m1, m2, m3, m4, m5, eps, keep_m, m4) : recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
+    return hp + hm;
 }
 
 // ------------------------------------------------------------------------------------------ Steger-Warming

@@ -196,6 +196,38 @@ def test_rhs_parity_eighth_order_viscous_scheme(B, Oracle, which):
     assert rel_linf(ref, ref6, U, floor).max() > 1e-9
 
 
+@pytest.mark.parametrize("which", ["plate", "ramp", "ramp3level", "box-ud7", "box-weno7", "box-weno5"])
+def test_rhs_parity_paper_boundary_scheme(B, Oracle, which):
+    """bc_closure = 1: shielded WENO5 next to aperiodic faces, in all three
+    sweep kernels (x tile kernel, y / z marching kernels); sizes leave ragged tiles at the far boundaries."""
+    if which == "plate":
+        case = W.flat_plate(nx=72, ny=44, nz=24)
+    elif which.startswith("ramp"):
+        case = W.ramp(nx=64, ny=44, nz=24, nmodes=12, theta2=np.inf if which == "ramp" else 0.1)
+    else:
+        case = W.smooth_periodic(70, 45, 23, grid="wavy", scheme=which.split("-")[1], Re=150.0, seed=6)
+        case.bc = ["outflow"] * 6          # every axis aperiodic: closures of all three sweeps and both ends
+    case.bc_closure = 1
+    got, ref, U = run_rhs_both(B, Oracle, case)
+    floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
+    err = rel_linf(got, ref, U, floor)
+    print(which, "rel Linf per component", err)
+    assert err.max() <= TOL_RHS
+    case.bc_closure = 0                # and the closure really changes the result
+    o = Oracle(case)
+    ref0 = o.rhs(o.fill_ghosts(case.U0.copy()))[INT]
+    assert np.abs(ref - ref0).max() > 1e-6 * np.abs(ref0).max()
+
+
+def test_twenty_steps_paper_boundary_scheme(B, Oracle):
+    case = W.flat_plate(nx=64, ny=40, nz=16)
+    case.bc_closure = 1
+    err, got, ref = step_both(B, Oracle, case, 20)
+    print("plate, paper's boundary scheme, 20 steps: rel Linf", err)
+    assert err <= 1e-9
+    assert np.isfinite(got).all()
+
+
 def test_ten_steps_eighth_order_viscous_scheme(B, Oracle):
     case = W.tgv(24, nsteps=10)
     case.visc_order = 8
