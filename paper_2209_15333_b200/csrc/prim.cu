@@ -8,20 +8,41 @@ namespace {
 // hold whatever the caller left there; their primitives are computed but never read.
 __global__ void __launch_bounds__(256) k_prim(long long np, GasDesc gs, const double *__restrict__ U,
                                               double *__restrict__ prim) {
-    long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x; id < np; id += stride) {
-        // true divisions (not a reciprocal multiply): this kernel is HBM-bound, and the pressure that feeds
-        // the shock-sensor decisions then rounds exactly as the definition does
-        double rho = U[id];
-        double u = U[np + id] / rho, v = U[2 * np + id] / rho, w = U[3 * np + id] / rho;
-        double p = gs.gm1 * (U[4 * np + id] - 0.5 * rho * (u * u + v * v + w * w));
-        double T = gs.gM2 * p / rho;
-        prim[P_U * np + id] = u;
-        prim[P_V * np + id] = v;
-        prim[P_W * np + id] = w;
-        prim[P_T * np + id] = T;
-        prim[P_C * np + id] = sqrt(T) * gs.invMa;
-        prim[P_P * np + id] = p;
+    // two consecutive points per thread as 16-byte accesses (np is even: nx is), two pairs in flight per thread
+    const long long npair = np >> 1, stride = (long long)gridDim.x * blockDim.x;
+    const double2 *U2 = reinterpret_cast<const double2 *>(U);
+    double2 *P2 = reinterpret_cast<double2 *>(prim);
+    for (long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x; id < npair; id += 2 * stride) {
+        double2 q[2][5];
+        bool ok[2];
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            ok[e] = id + e * stride < npair;
+            if (ok[e]) {
+#pragma unroll
+                for (int m = 0; m < 5; ++m) q[e][m] = __ldcs(U2 + m * npair + id + e * stride);
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            if (!ok[e]) continue;
+            double2 u, v, w, p, T, c;
+            // true divisions (not a reciprocal multiply): this kernel is HBM-bound, and the pressure that feeds
+            // the shock-sensor decisions then rounds exactly as the definition does
+            u.x = q[e][1].x / q[e][0].x; v.x = q[e][2].x / q[e][0].x; w.x = q[e][3].x / q[e][0].x;
+            u.y = q[e][1].y / q[e][0].y; v.y = q[e][2].y / q[e][0].y; w.y = q[e][3].y / q[e][0].y;
+            p.x = gs.gm1 * (q[e][4].x - 0.5 * q[e][0].x * (u.x * u.x + v.x * v.x + w.x * w.x));
+            p.y = gs.gm1 * (q[e][4].y - 0.5 * q[e][0].y * (u.y * u.y + v.y * v.y + w.y * w.y));
+            T.x = gs.gM2 * p.x / q[e][0].x; T.y = gs.gM2 * p.y / q[e][0].y;
+            c.x = sqrt(T.x) * gs.invMa; c.y = sqrt(T.y) * gs.invMa;
+            const long long o = id + e * stride;
+            P2[P_U * npair + o] = u;
+            P2[P_V * npair + o] = v;
+            P2[P_W * npair + o] = w;
+            P2[P_T * npair + o] = T;
+            P2[P_C * npair + o] = c;
+            P2[P_P * npair + o] = p;
+        }
     }
 }
 
@@ -154,8 +175,9 @@ __global__ void __launch_bounds__(256) k_wavespeed(GridDesc g, GasDesc gs, const
 
 ocfd_status launch_prim(ocfd_ctx *c, const double *U) {
     long long np = c->g.np;
-    int blocks = (int)((np + 255) / 256);
-    if (blocks > 148 * 32) blocks = 148 * 32;
+    int blocks = (int)((np / 4 + 255) / 256);   // a thread takes two pairs of points per pass
+    if (blocks < 1) blocks = 1;
+    if (blocks > c->nsm * 16) blocks = c->nsm * 16;
     OCFD_T0(c, K_PRIM);
     k_prim<<<blocks, 256, 0, c->stream>>>(np, c->gas, U, c->prim);
     OCFD_CHECK_LAUNCH(c);
