@@ -1,5 +1,6 @@
 // Rows a2 (primitives), a3 (shock sensor) and a9 (max wavespeed).
 #include "ocfd_internal.cuh"
+#include "schemes.cuh"
 #include "tma.cuh"
 
 namespace {
@@ -98,14 +99,15 @@ __global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, const __grid_constan
             const double nj = fabs(t0 - c[-SBX] - c[SBX]), dj = t0 + c[-SBX] + c[SBX];
             const double nk = fabs(t0 - pm - pp), dk = t0 + pm + pp;
             const double dij = di * dj;
-            const double th = (ni * (dj * dk) + nj * (di * dk) + nk * dij) / (dij * dk);
+            const double th = fast_div_pos(ni * (dj * dk) + nj * (di * dk) + nk * dij, dij * dk);
             const long long id = pidx(g, i + OCFD_NG, j + OCFD_NG, k + OCFD_NG);
             theta[id] = th;
             const int cc[3] = {i, j, k};
             const int n[3] = {g.nx, g.ny, g.nz};
             const long long st[3] = {1, g.sy, g.sz};
+            const bool face = i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1;
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
+            for (int d = 0; d < 3 && face; ++d) {
                 if (cc[d] == 0) theta[g.periodic[d] ? id + n[d] * st[d] : id - st[d]] = th;
                 if (cc[d] == n[d] - 1) theta[g.periodic[d] ? id - n[d] * st[d] : id + st[d]] = th;
             }

@@ -10,6 +10,7 @@
 // window per thread; the x / y neighbours of the current plane are read from the staged box (3-point halos; the box is
 // 4 wider in x on each side because a TMA box of doubles must start at an even x index).
 #include "ocfd_internal.cuh"
+#include "schemes.cuh"
 #include "tma.cuh"
 
 namespace {
@@ -163,7 +164,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
                 gz[a] = m[0][2] * gr[a][0] + m[1][2] * gr[a][1] + m[2][2] * gr[a][2];
             }
             const double T = w[0][H], u = w[1][H], v = w[2][H], ww = w[3][H];
-            const double mu0 = (1.0 + gs.suth) / (T + gs.suth) * T * sqrt(T);  // eq. 15
+            const double mu0 = fast_div_pos((1.0 + gs.suth) * (T * sqrt(T)), T + gs.suth);  // eq. 15
             const double mu = mu0 * gs.invRe, kc = mu0 * gs.kfac;              // eq. 14
             const double div = gx[1] + gy[2] + gz[3];
             const double txx = mu * (2.0 * gx[1] - (2.0 / 3.0) * div);         // eq. 13
