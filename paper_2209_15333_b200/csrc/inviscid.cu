@@ -327,12 +327,16 @@ bool encode_maps(ocfd_ctx *c, const double *U, double *dU) {
 
 // dU <- -J sum_d (h_{s+1/2} - h_{s-1/2}); the x sweep writes, y and z accumulate (same order as the definition)
 ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU) {
-    if (!encode_maps(c, U, dU)) return OCFD_ECUDA;
     ocfd_status st;
-    switch (c->g.kind) {
-        case OCFD_GRID_UNIFORM: st = launch_kind<OCFD_GRID_UNIFORM>(c); break;
-        case OCFD_GRID_STRETCHED: st = launch_kind<OCFD_GRID_STRETCHED>(c); break;
-        default: st = launch_kind<OCFD_GRID_CURVILINEAR>(c);
+    if (c->x_tile) {
+        if (!encode_maps(c, U, dU)) return OCFD_ECUDA;
+        switch (c->g.kind) {
+            case OCFD_GRID_UNIFORM: st = launch_kind<OCFD_GRID_UNIFORM>(c); break;
+            case OCFD_GRID_STRETCHED: st = launch_kind<OCFD_GRID_STRETCHED>(c); break;
+            default: st = launch_kind<OCFD_GRID_CURVILINEAR>(c);
+        }
+    } else {
+        st = launch_inviscid_march(c, U, dU, 0);
     }
     if (st != OCFD_OK) return st;
     if ((st = launch_inviscid_march(c, U, dU, 1)) != OCFD_OK) return st;

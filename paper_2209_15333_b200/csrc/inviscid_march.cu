@@ -38,21 +38,24 @@ struct JRow {
     const double *p;   // curvilinear: J of row 0 of the pencil; stretched: the 1-D metric of the sweep axis
     long long st;      // curvilinear: row stride
     double f0, f1;     // stretched: the two fixed 1-D metrics
-    __device__ __forceinline__ JRow(const GridDesc &g, int ip, int crossp) : p(nullptr), st(0), f0(0.0), f1(0.0) {
+    // ap = padded across index (y for the x sweep, else x), crossp = padded cross index (z, z, y for DIR 0, 1, 2)
+    __device__ __forceinline__ JRow(const GridDesc &g, int ap, int crossp) : p(nullptr), st(0), f0(0.0), f1(0.0) {
         if (KIND == OCFD_GRID_STRETCHED) {
-            f0 = __ldg(g.met[0] + ip);
-            f1 = __ldg(g.met[DIR == 1 ? 8 : 4] + crossp);
-            p = g.met[DIR == 1 ? 4 : 8];
+            f0 = __ldg(g.met[DIR == 0 ? 4 : 0] + ap);
+            f1 = __ldg(g.met[DIR == 2 ? 4 : 8] + crossp);
+            p = g.met[4 * DIR];
         } else if (KIND == OCFD_GRID_CURVILINEAR) {
-            st = DIR == 1 ? g.sy : g.msk;
-            p = g.atab[0] + 4 * g.atab_fs + (DIR == 1 ? (long long)crossp * g.msk : (long long)crossp * g.sy) + ip;
+            st = DIR == 0 ? 1 : DIR == 1 ? g.sy : g.msk;
+            p = g.atab[0] + 4 * g.atab_fs +
+                (DIR == 0 ? (long long)crossp * g.msk + (long long)ap * g.sy
+                          : (DIR == 1 ? (long long)crossp * g.msk : (long long)crossp * g.sy) + ap);
         }
     }
     __device__ __forceinline__ double at(const GridDesc &g, int i0, int e) const {
         if (KIND == OCFD_GRID_UNIFORM) return g.uJ;
         if (KIND == OCFD_GRID_STRETCHED) {
             const double m = __ldg(p + i0 + e);
-            return DIR == 1 ? (f0 * m) * f1 : (f0 * f1) * m;   // (xi_x eta_y) zeta_z
+            return DIR == 0 ? (m * f0) * f1 : DIR == 1 ? (f0 * m) * f1 : (f0 * f1) * m;   // (xi_x eta_y) zeta_z
         }
         return __ldg(p + (long long)(i0 + e) * st);
     }
@@ -73,7 +76,12 @@ __device__ __forceinline__ double recon_pair(int flag, double p0, double p1, dou
     return recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps) + recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
 }
 
-// KIND: grid kind, SCHEME: ocfd_scheme, DIR: 1 y, 2 z.  grid = (tiles across x, cross extent)
+// KIND: grid kind, SCHEME: ocfd_scheme, DIR: 0 x, 1 y, 2 z.  grid = (tiles across, cross extent).
+// DIR 0: the 32 pencils are 32 consecutive y lines and a chunk is 4 x-points of each (boxes of 32-byte rows; the tensor
+// maps of the x sweep ask the L2 for 256-byte fills, so that the 8 chunks that share them find them there).  The
+// shared arrays keep the box order (x fastest), the split fluxes are stored with an XOR swizzle of the pencil index so
+// that both the point-wise phase and the walkers are free of bank conflicts, and the output tile is written as two
+// 16-byte stores per walker and leaves by a TMA store (the x sweep writes dU, y and z accumulate).
 template <int KIND, int SCHEME, int DIR>
 __global__ void __launch_bounds__(MNT, 4)
     k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
@@ -90,25 +98,25 @@ __global__ void __launch_bounds__(MNT, 4)
 
     const int tid = threadIdx.x;
     const int a0 = blockIdx.x * MAC, cross = blockIdx.y;
-    const int nd = DIR == 1 ? g.ny : g.nz;
+    const int nd = DIR == 0 ? g.nx : DIR == 1 ? g.ny : g.nz;
+    const int nap = DIR == 0 ? g.nyp : g.nxp;   // padded extent across
     const int ndp = nd + 2 * OCFD_NG;
     const int nch = (ndp + MR - 1) / MR;
 
     auto issue = [&](int c) {   // one thread: boxes of chunk c (padded rows MR*c ..) towards stage c % MNST
         const int s = c % MNST;
         double *dst = sIn + s * MSTG;
-        const int c0 = OCFD_NG + a0;
-        const int c1 = DIR == 1 ? MR * c : OCFD_NG + cross;
+        const int c0 = DIR == 0 ? MR * c : OCFD_NG + a0;
+        const int c1 = DIR == 0 ? OCFD_NG + a0 : DIR == 1 ? MR * c : OCFD_NG + cross;
         const int c2 = DIR == 2 ? MR * c : OCFD_NG + cross;
         // curvilinear grids: the metric tables k1, k2, k3, sigma and J of the chunk come the same way (mfull = 0: a
         // z-extruded map swept along z, one row serves the whole chunk)
         const uint32_t mbytes = KIND == OCFD_GRID_CURVILINEAR ? 5u * (mfull ? MPTS : MAC) * 8u : 0u;
         tma::mbar_expect_tx(&bars[s], (SCHEME == OCFD_HYBRID ? 6 : 5) * MPTS * 8 + mbytes);
         if (KIND == OCFD_GRID_CURVILINEAR) {
-            const int m1 = DIR == 1 ? MR * c : OCFD_NG + cross;
-            const int m2 = DIR == 1 ? (g.msk ? OCFD_NG + cross : 0) : (mfull ? MR * c : 0);
-            tma::load4(dst + 6 * MPTS, &tm_met, &bars[s], c0, m1, m2, 0);
-            tma::load4(sJ + (c % MNJ) * MPTS, &tm_metJ, &bars[s], c0, m1, m2, 4);
+            const int m2 = DIR == 2 ? (mfull ? MR * c : 0) : (g.msk ? OCFD_NG + cross : 0);
+            tma::load4(dst + 6 * MPTS, &tm_met, &bars[s], c0, c1, m2, 0);
+            tma::load4(sJ + (c % MNJ) * MPTS, &tm_metJ, &bars[s], c0, c1, m2, 4);
         }
         tma::load4(dst, &tm_rho, &bars[s], c0, c1, c2, 0);
         tma::load4(dst + MPTS, &tm_prim, &bars[s], c0, c1, c2, P_U);
@@ -123,12 +131,14 @@ __global__ void __launch_bounds__(MNT, 4)
     }
 
     // phase A role: point (row pr, pencil pa) of every chunk; walker role: pencil wa, component wm
-    const int pr = tid / MAC, pa = tid % MAC;
+    // (in both cases the point of thread tid sits at position tid of a staged box)
+    const int pr = DIR == 0 ? tid % MR : tid / MAC, pa = DIR == 0 ? (tid / MR) % MAC : tid % MAC;
     const bool producer = tid < MPTS;
-    const int wa = pa, wm = pr;
-    const int ipA = OCFD_NG + a0 + pa;
-    const bool x_ok = ipA < g.nxp - OCFD_NG;   // pencils past the last interior x hold zero-filled state
-    const JRow<KIND, DIR> jrow(g, min(ipA, g.nxp - 1), OCFD_NG + cross);
+    const int wa = tid % MAC, wm = tid / MAC;
+    const int apA = OCFD_NG + a0 + pa;
+    const bool x_ok = apA < nap - OCFD_NG;   // pencils past the last interior line hold zero-filled state
+    const JRow<KIND, DIR> jrow(g, min(OCFD_NG + a0 + wa, nap - 1), OCFD_NG + cross);
+    const int sfi = DIR == 0 ? pr * MAC + (pa ^ (pr << 2)) : tid;   // this thread's point inside a split-flux field
 
     // Register windows as rings of 8: padded row r lives in slot r % 8.  Two chunks (8 rows) bring every slot back to
     // its place, so the chunk loop is unrolled by two and no value is ever moved between registers.
@@ -151,8 +161,8 @@ __global__ void __launch_bounds__(MNT, 4)
         const int rowA = r0 + pr;
         const bool validA = producer && x_ok && rowA < ndp;
         if (KIND != OCFD_GRID_CURVILINEAR && validA)
-            met_ksJ<KIND, DIR>(g, ipA, DIR == 1 ? rowA : OCFD_NG + cross, DIR == 2 ? rowA : OCFD_NG + cross, k1, k2, k3, sig,
-                               Jdead);
+            met_ksJ<KIND, DIR>(g, DIR == 0 ? rowA : apA, DIR == 0 ? apA : DIR == 1 ? rowA : OCFD_NG + cross,
+                               DIR == 2 ? rowA : OCFD_NG + cross, k1, k2, k3, sig, Jdead);
         // ... and J of the four points this walker completes in this chunk (padded rows r0-4 .. r0-1; the first
         // chunk completes nothing that is kept)
         double Jw[MR];
@@ -169,14 +179,14 @@ __global__ void __launch_bounds__(MNT, 4)
                 const double *mp = sU + 6 * MPTS + mi;
                 k1 = mp[0]; k2 = mp[mfs]; k3 = mp[2 * mfs]; sig = mp[3 * mfs];
             }
-            const double *jp = sJ + ((c + MNJ - 1) % MNJ) * MPTS + wa;   // arrived with chunk c-1 (rows r0-4 .. r0-1)
+            const double *jp = sJ + ((c + MNJ - 1) % MNJ) * MPTS;   // arrived with chunk c-1 (rows r0-4 .. r0-1)
 #pragma unroll
-            for (int e = 0; e < MR; ++e) Jw[e] = jp[mfull ? e * MAC : 0];
+            for (int e = 0; e < MR; ++e) Jw[e] = DIR == 0 ? jp[wa * MR + e] : jp[(mfull ? e * MAC : 0) + wa];
         }
 
         // ---- phase A: split fluxes of the chunk's points; pf(r) = scheme flag of the interface between rows r-1, r
         if (producer) {
-            double *dst = sF + tid;
+            double *dst = sF + sfi;
             if (validA) {
                 sw_split_store<KIND, DIR>(gs, sU[tid], sU[MPTS + tid], sU[2 * MPTS + tid], sU[3 * MPTS + tid],
                                           sU[4 * MPTS + tid], k1, k2, k3, sig, dst, MPTS);
@@ -187,8 +197,9 @@ __global__ void __launch_bounds__(MNT, 4)
             if (SCHEME == OCFD_HYBRID) {
                 unsigned char f = 0;
                 if (rowA >= OCFD_NG && rowA <= nd + OCFD_NG) {   // interfaces -1/2 .. nd-1/2 (eq. 42, R-12)
-                    const double *thp = pr > 0 ? sU + 5 * MPTS + tid - MAC
-                                               : sIn + ((c + MNST - 1) % MNST) * MSTG + 5 * MPTS + (MR - 1) * MAC + pa;
+                    const double *thp =
+                        pr > 0 ? sU + 5 * MPTS + tid - (DIR == 0 ? 1 : MAC)
+                               : sIn + ((c + MNST - 1) % MNST) * MSTG + 5 * MPTS + (DIR == 0 ? tid + MR - 1 : (MR - 1) * MAC + pa);
                     f = (unsigned char)iface_flag(gs, *thp, sU[5 * MPTS + tid]);
                 }
                 sFl[4 * pa + pr] = f;
@@ -200,8 +211,9 @@ __global__ void __launch_bounds__(MNT, 4)
 
         // ---- phase B: push the chunk's rows through the register windows
         // pushing row r completes interface (r-4)+1/2 (f+ rows r-7..r-1, f- rows r-6..r) and with it point r-4
-        double *so = sO + PH * 5 * MPTS + wm * MPTS + wa;
-        const double *fpn = sF + wm * MPTS + wa, *fmn = sF + (wm + 5) * MPTS + wa;
+        double *so = sO + PH * 5 * MPTS + wm * MPTS + (DIR == 0 ? wa * MR : wa);
+        const double *fpn = sF + wm * MPTS, *fmn = sF + (wm + 5) * MPTS;
+        double out[MR];
         bool fast = SCHEME == OCFD_UD7;
         unsigned cur = 0;
         if (SCHEME == OCFD_HYBRID) {
@@ -219,8 +231,9 @@ __global__ void __launch_bounds__(MNT, 4)
         double nP[MR], nM[MR];   // the chunk's new rows (loaded up front, entered into the rings one by one)
 #pragma unroll
         for (int e = 0; e < MR; ++e) {
-            nP[e] = fpn[e * MAC];
-            nM[e] = fmn[e * MAC];
+            const int q = e * MAC + (DIR == 0 ? wa ^ (e << 2) : wa);
+            nP[e] = fpn[q];
+            nM[e] = fmn[q];
         }
         if (fast) {
 #pragma unroll
@@ -232,7 +245,8 @@ __global__ void __launch_bounds__(MNT, 4)
                                      Wp[(k + 6) & 7], Wp[(k + 7) & 7]) +
                                  ud7(Wm[k & 7], Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
                                      Wm[(k + 3) & 7], Wm[(k + 2) & 7]);
-                so[e * MAC] = -Jw[e] * (h - hprev);
+                if (DIR == 0) out[e] = -Jw[e] * (h - hprev);
+                else so[e * MAC] = -Jw[e] * (h - hprev);
                 hprev = h;
             }
         } else {
@@ -252,15 +266,21 @@ __global__ void __launch_bounds__(MNT, 4)
                                                   Wp[(k + 5) & 7], Wp[(k + 6) & 7], Wp[(k + 7) & 7], Wm[k & 7],
                                                   Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
                                                   Wm[(k + 3) & 7], Wm[(k + 2) & 7], gs.weno_eps);
-                so[e * MAC] = -Jw[e] * (h - hprev);
+                if (DIR == 0) out[e] = -Jw[e] * (h - hprev);
+                else so[e * MAC] = -Jw[e] * (h - hprev);
                 hprev = h;
             }
+        }
+        if (DIR == 0) {
+            reinterpret_cast<double2 *>(so)[0] = make_double2(out[0], out[1]);
+            reinterpret_cast<double2 *>(so)[1] = make_double2(out[2], out[3]);
         }
         tma::fence_proxy_async();
         __syncthreads();
         if (tid == 0 && r0 + MR - 1 >= 2 * OCFD_NG) {
             const int o = r0 - 2 * OCFD_NG;   // interior index of the first completed point (negative rows are clipped)
-            tma::reduce_add4(&tm_out, sO + PH * 5 * MPTS, a0, DIR == 1 ? o : cross, DIR == 2 ? o : cross, 0);
+            if (DIR == 0) tma::store4(&tm_out, sO + PH * 5 * MPTS, o, a0, cross, 0);
+            else tma::reduce_add4(&tm_out, sO + PH * 5 * MPTS, a0, DIR == 1 ? o : cross, DIR == 2 ? o : cross, 0);
             tma::store_commit();
             tma::store_wait_read<1>();   // the other output tile is free for the next chunk
         }
@@ -283,12 +303,12 @@ ocfd_status launch_march(ocfd_ctx *c) {
             return OCFD_ECUDA;
         attr_set = true;
     }
-    const int ncross = DIR == 1 ? g.nz : g.ny;
+    const int ncross = DIR == 2 ? g.ny : g.nz;
     if (ncross > 65535) return OCFD_EINVAL;
-    dim3 grd((g.nx + MAC - 1) / MAC, ncross, 1);
+    dim3 grd(((DIR == 0 ? g.ny : g.nx) + MAC - 1) / MAC, ncross, 1);
     OCFD_T0(c, K_INV_X + DIR);
     const MarchMaps &M = c->march;
-    const int mfull = DIR == 1 || g.msk != 0;
+    const int mfull = DIR != 2 || g.msk != 0;
     k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.rho[DIR], M.prim[DIR], M.th[DIR],
                                                                         M.out[DIR], M.met[DIR], M.metJ[DIR], mfull);
     OCFD_CHECK_LAUNCH(c);
@@ -297,7 +317,7 @@ ocfd_status launch_march(ocfd_ctx *c) {
 
 template <int KIND, int SCHEME>
 ocfd_status launch_march_dir(ocfd_ctx *c, int dir) {
-    return dir == 1 ? launch_march<KIND, SCHEME, 1>(c) : launch_march<KIND, SCHEME, 2>(c);
+    return dir == 0 ? launch_march<KIND, SCHEME, 0>(c) : dir == 1 ? launch_march<KIND, SCHEME, 1>(c) : launch_march<KIND, SCHEME, 2>(c);
 }
 
 template <int KIND>
@@ -316,24 +336,24 @@ bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
     MarchMaps &M = c->march;
     const long long full1[4] = {g.nxp, g.nyp, g.nzp, 1}, full6[4] = {g.nxp, g.nyp, g.nzp, P_NF};
     const long long inner[4] = {g.nx, g.ny, g.nz, 5};
-    for (int d = 1; d < 3; ++d) {
-        const int by = d == 1 ? MR : 1, bz = d == 2 ? MR : 1;
-        const int b1[4] = {MAC, by, bz, 1}, b4[4] = {MAC, by, bz, 4}, bo[4] = {MAC, by, bz, 5};
+    for (int d = 0; d < 3; ++d) {
+        const int bx = d == 0 ? MR : MAC, by = d == 0 ? MAC : d == 1 ? MR : 1, bz = d == 2 ? MR : 1;
+        const int b1[4] = {bx, by, bz, 1}, b4[4] = {bx, by, bz, 4}, bo[4] = {bx, by, bz, 5};
         if (!M.ready) {
             if (g.kind == OCFD_GRID_CURVILINEAR) {
                 // the derived metric table of this direction: [5][planes][nyp][nxp], one plane if z-extruded
                 const long long mdim[4] = {g.nxp, g.nyp, g.msk ? g.nzp : 1, 5};
                 const int mz = d == 2 && g.msk ? MR : 1;
-                const int m4[4] = {MAC, by, mz, 4}, m1[4] = {MAC, by, mz, 1};
-                if (!ocfd_tma_encode(&M.met[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m4)) return false;
-                if (!ocfd_tma_encode(&M.metJ[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m1)) return false;
+                const int m4[4] = {bx, by, mz, 4}, m1[4] = {bx, by, mz, 1};
+                if (!ocfd_tma_encode(&M.met[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m4, d == 0)) return false;
+                if (!ocfd_tma_encode(&M.metJ[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m1, d == 0)) return false;
             } else {   // unused, but the kernel takes the parameters
                 M.met[d] = M.metJ[d] = CUtensorMap();
             }
-            if (!ocfd_tma_encode(&M.prim[d], c->prim, full6, g.sy, g.sz, g.np, b4)) return false;
-            if (!ocfd_tma_encode(&M.th[d], c->theta, full1, g.sy, g.sz, g.np, b1)) return false;
+            if (!ocfd_tma_encode(&M.prim[d], c->prim, full6, g.sy, g.sz, g.np, b4, d == 0)) return false;
+            if (!ocfd_tma_encode(&M.th[d], c->theta, full1, g.sy, g.sz, g.np, b1, d == 0)) return false;
         }
-        if (M.U != U && !ocfd_tma_encode(&M.rho[d], U, full1, g.sy, g.sz, g.np, b1)) return false;
+        if (M.U != U && !ocfd_tma_encode(&M.rho[d], U, full1, g.sy, g.sz, g.np, b1, d == 0)) return false;
         if (M.dU != dU &&
             !ocfd_tma_encode(&M.out[d], dU + (long long)OCFD_NG * (g.sz + g.sy + 1), inner, g.sy, g.sz, g.np, bo))
             return false;
@@ -347,7 +367,7 @@ bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
 }  // namespace
 
 ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int dir) {
-    if (dir != 1 && dir != 2) return OCFD_EINVAL;
+    if (dir < 0 || dir > 2) return OCFD_EINVAL;
     if (!encode_march_maps(c, U, dU)) return OCFD_ECUDA;
     switch (c->g.kind) {
         case OCFD_GRID_UNIFORM: return launch_march_kind<OCFD_GRID_UNIFORM>(c, dir);

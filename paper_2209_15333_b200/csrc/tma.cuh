@@ -36,8 +36,9 @@ inline ocfd_encode_fn ocfd_tma_encoder() {
 
 // Rank-4 fp64 tensor map: extents dim[4] (x,y,z,field), strides in doubles of y, z, field; box[4].
 // Returns false when the driver rejects the description.
+// wide_fill: ask the L2 to fill 256 bytes around every request (boxes with short rows that neighbours in time complete).
 inline bool ocfd_tma_encode(CUtensorMap *tm, const double *base, const long long dim[4], long long sy, long long sz,
-                            long long sf, const int box[4]) {
+                            long long sf, const int box[4], bool wide_fill = false) {
     ocfd_encode_fn enc = ocfd_tma_encoder();
     if (!enc) return false;
     cuuint64_t gd[4] = {(cuuint64_t)dim[0], (cuuint64_t)dim[1], (cuuint64_t)dim[2], (cuuint64_t)dim[3]};
@@ -45,7 +46,8 @@ inline bool ocfd_tma_encode(CUtensorMap *tm, const double *base, const long long
     cuuint32_t bx[4] = {(cuuint32_t)box[0], (cuuint32_t)box[1], (cuuint32_t)box[2], (cuuint32_t)box[3]};
     cuuint32_t es[4] = {1, 1, 1, 1};
     return enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+               CU_TENSOR_MAP_SWIZZLE_NONE, wide_fill ? CU_TENSOR_MAP_L2_PROMOTION_L2_256B : CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // ------------------------------------------------------------------------------------------------ device side
