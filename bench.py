@@ -193,6 +193,23 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def max_over_ranks(x, world, device="cpu"):
+    """Max of a per-rank scalar over all ranks (NCCL on the GPU box, gloo in the CPU tests); identity for one rank."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(seconds_local, points_per_rank, steps, world, device="cpu"):
+    """Replicas only (DESIGN section 1): every rank advances its own copy of the workload, no data-path collective;
+    the job's throughput is all ranks' grid-point steps over the slowest rank's time."""
+    return world * points_per_rank * steps / max_over_ranks(seconds_local, world, device)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -246,11 +263,8 @@ def run_ours(args):
     per_kernel = s.timing_read()
     s.timing(False)
     finite = bool(torch.isfinite(U).all().item())
-    tmax = torch.tensor([ms], dtype=torch.float64, device=s.device)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_all = float(tmax.item())
-    value = world * case.npoints * args.steps / (ms_all * 1e-3)
+    ms_all = max_over_ranks(ms, world, s.device)
+    value = whole_job_value(ms * 1e-3, case.npoints, args.steps, world, s.device)
 
     # ---- end to end through the C ABI with HOST buffers: H2D + step + D2H inside the timed region, every step
     n_e2e = max(1, min(args.steps, 3))
@@ -263,10 +277,7 @@ def run_ours(args):
         s.rk3_steps_host(Uh, U, dt, 1)      # synchronises the stream before returning
     barrier()
     t_e2e = time.perf_counter() - t0
-    te = torch.tensor([t_e2e], dtype=torch.float64, device=s.device)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * case.npoints * n_e2e / float(te.item())
+    e2e_value = whole_job_value(t_e2e, case.npoints, n_e2e, world, s.device)
     nbytes = int(Uh.numel() * 8)
 
     if rank != 0:
