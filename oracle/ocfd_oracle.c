@@ -66,6 +66,7 @@ typedef struct {
                                 PAPER.md:L313 "two such schemes, of sixth and eighth order" */
     int bc_closure;          /* 0: ghost cells feed the full stencils (north_star; DESIGN R-14);
                                 1: the paper's boundary scheme, PAPER.md:L307-309 (DESIGN R-20, R-21) */
+    int char_recon;          /* 1: flux reconstruction in characteristic variables, PAPER.md:L212-263 (section 2.2.2) */
 } ora_params;
 static int vorder(const ora_params *P) { return P->visc_order == 8 ? 8 : 6; }
 
@@ -465,6 +466,80 @@ static void iface_flux(int scheme, double eps, const double fp[8][5], const doub
         h[m] = hp + hm;
     }
 }
+/* ---------------------------------- reconstruction in characteristic variables (section 2.2.2) */
+/* Left / right eigenvector matrices S (eq. 35) and S^-1 (eq. 34) of the flux Jacobian in the unit direction n, for
+ * the state (u, v, w, c); V = q^2/2 (eq. 25), H = V + c^2/(gamma-1), kappa = (gamma-1)/c^2, kappa1 = kappa/2,
+ * chi = 1/(2c) (eq. 36); l by eq. 39, m = n x l (eq. 40). */
+void ora_eigen_matrices(double gamma, double u, double v, double w, double c, const double n[3], double S[5][5],
+                        double Si[5][5]) {
+    double l[3], m[3];
+    if (fabs(n[2]) <= fabs(n[1])) {
+        double r = sqrt(n[0] * n[0] + n[1] * n[1]);
+        l[0] = -n[1] / r; l[1] = n[0] / r; l[2] = 0.0;
+    } else {
+        double r = sqrt(n[0] * n[0] + n[2] * n[2]);
+        l[0] = -n[2] / r; l[1] = 0.0; l[2] = n[0] / r;
+    }
+    m[0] = n[1] * l[2] - n[2] * l[1]; m[1] = n[2] * l[0] - n[0] * l[2]; m[2] = n[0] * l[1] - n[1] * l[0];
+    const double V = 0.5 * (u * u + v * v + w * w), H = V + c * c / (gamma - 1.0);
+    const double un = u * n[0] + v * n[1] + w * n[2], ul = u * l[0] + v * l[1] + w * l[2], um = u * m[0] + v * m[1] + w * m[2];
+    const double kap = (gamma - 1.0) / (c * c), k1 = 0.5 * kap, chi = 1.0 / (2.0 * c);
+    const double vel[3] = { u, v, w };
+    /* S^-1: columns are the right eigenvectors (eq. 34) */
+    Si[0][0] = 1.0; Si[0][1] = 0.0; Si[0][2] = 0.0; Si[0][3] = 1.0; Si[0][4] = 1.0;
+    for (int r = 0; r < 3; ++r) {
+        Si[r + 1][0] = vel[r]; Si[r + 1][1] = l[r]; Si[r + 1][2] = m[r];
+        Si[r + 1][3] = vel[r] - c * n[r]; Si[r + 1][4] = vel[r] + c * n[r];
+    }
+    Si[4][0] = V; Si[4][1] = ul; Si[4][2] = um; Si[4][3] = H - c * un; Si[4][4] = H + c * un;
+    /* S: rows are the left eigenvectors (eq. 35) */
+    S[0][0] = 1.0 - kap * V; S[0][4] = -kap;
+    S[1][0] = -ul; S[1][4] = 0.0;
+    S[2][0] = -um; S[2][4] = 0.0;
+    S[3][0] = k1 * V + chi * un; S[3][4] = k1;
+    S[4][0] = k1 * V - chi * un; S[4][4] = k1;
+    for (int r = 0; r < 3; ++r) {
+        S[0][r + 1] = kap * vel[r];
+        S[1][r + 1] = l[r];
+        S[2][r + 1] = m[r];
+        S[3][r + 1] = -chi * n[r] - k1 * vel[r];
+        S[4][r + 1] = chi * n[r] - k1 * vel[r];
+    }
+}
+/* S, S^-1 of interface s+1/2 along d: state from the simple average of the conserved variables of its two points
+ * (eq. 32); direction n = (alpha_s + alpha_s+1) normalised, alpha = grad(d)/J (the paper does not say where the
+ * metrics of the interface come from: DESIGN R-22). */
+static void iface_eigen(const ora_params *P, const double *U, int d, const int c0[3], double S[5][5], double Si[5][5]) {
+    int c1[3] = { c0[0], c0[1], c0[2] };
+    c1[d] += 1;
+    long np = NP(P), ia = IDX(P, c0[0], c0[1], c0[2]), ib = IDX(P, c1[0], c1[1], c1[2]);
+    double Ua[5], n[3] = { 0, 0, 0 };
+    for (int m = 0; m < 5; ++m) Ua[m] = 0.5 * (U[m * np + ia] + U[m * np + ib]);
+    ora_prim q = prim_of(P, Ua[0], Ua[1], Ua[2], Ua[3], Ua[4]);
+    long ma = MIDX(P, c0[0], c0[1], c0[2]), mb = MIDX(P, c1[0], c1[1], c1[2]);
+    for (int r = 0; r < 3; ++r) n[r] = P->met[3 * d + r][ma] / P->met[9][ma] + P->met[3 * d + r][mb] / P->met[9][mb];
+    double len = sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+    for (int r = 0; r < 3; ++r) n[r] /= len;
+    ora_eigen_matrices(P->gamma, q.u, q.v, q.w, q.c, n, S, Si);
+}
+/* iface_flux in characteristic variables (eq. 31): the split fluxes of every stencil point are projected with the S
+ * of the interface, each characteristic component is reconstructed by the scheme, the sum is projected back. */
+static void iface_flux_char(int scheme, double eps, const double fp[8][5], const double fm[8][5], double h[5],
+                            int closure, int s, int n, const double S[5][5], const double Si[5][5]) {
+    double wp[8][5], wm[8][5], hw[5];
+    for (int r = 0; r < 8; ++r)
+        for (int k = 0; k < 5; ++k) {
+            double a = 0.0, b = 0.0;
+            for (int m = 0; m < 5; ++m) { a += S[k][m] * fp[r][m]; b += S[k][m] * fm[r][m]; }
+            wp[r][k] = a; wm[r][k] = b;
+        }
+    iface_flux(scheme, eps, (const double(*)[5])wp, (const double(*)[5])wm, hw, closure, s, n);
+    for (int m = 0; m < 5; ++m) {
+        double a = 0.0;
+        for (int k = 0; k < 5; ++k) a += Si[m][k] * hw[k];
+        h[m] = a;
+    }
+}
 static int closure_on(const ora_params *P, int d) { return P->bc_closure && !periodic(P, d); }
 /* dU -= J (h_{s+1/2} - h_{s-1/2}) over all interior points, direction d  (A.1, A.6) */
 static void inviscid_dir(const ora_params *P, const double *U, const double *theta, int d, double *dU) {
@@ -490,8 +565,15 @@ static void inviscid_dir(const ora_params *P, const double *U, const double *the
                     c[d] = s;
                     long id = IDX(P, c[0], c[1], c[2]);
                     int sch = P->scheme == ORA_HYBRID ? iface_scheme(P, theta[id], theta[id + dim_stride(P, d)]) : P->scheme;
-                    iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + (s - 3 + NG)), (const double(*)[5])(fm + (s - 3 + NG)), h[s + 1],
-                               closure_on(P, d), s, n);
+                    if (P->char_recon) {
+                        double S[5][5], Si[5][5];
+                        iface_eigen(P, U, d, c, S, Si);
+                        iface_flux_char(sch, P->weno_eps, (const double(*)[5])(fp + (s - 3 + NG)),
+                                        (const double(*)[5])(fm + (s - 3 + NG)), h[s + 1], closure_on(P, d), s, n,
+                                        (const double(*)[5])S, (const double(*)[5])Si);
+                    } else
+                        iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + (s - 3 + NG)),
+                                   (const double(*)[5])(fm + (s - 3 + NG)), h[s + 1], closure_on(P, d), s, n);
                 }
                 for (int s = 0; s < n; ++s) {
                     c[d] = s;
@@ -682,8 +764,16 @@ void ora_rhs_point(const ora_params *P, const double *U, int i, int j, int k, do
                 a[d] = s0 - 1 + e; b[d] = s0 + e;
                 sch = iface_scheme(P, theta_for(P, U, d, a[0], a[1], a[2]), theta_for(P, U, d, b[0], b[1], b[2]));
             }
-            iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + e), (const double(*)[5])(fm + e), h[e],
-                       closure_on(P, d), s0 - 1 + e, dim_n(P, d));
+            if (P->char_recon) {
+                double S[5][5], Si[5][5];
+                int ci[3] = { i, j, k };
+                ci[d] = s0 - 1 + e;
+                iface_eigen(P, U, d, ci, S, Si);
+                iface_flux_char(sch, P->weno_eps, (const double(*)[5])(fp + e), (const double(*)[5])(fm + e), h[e],
+                                closure_on(P, d), s0 - 1 + e, dim_n(P, d), (const double(*)[5])S, (const double(*)[5])Si);
+            } else
+                iface_flux(sch, P->weno_eps, (const double(*)[5])(fp + e), (const double(*)[5])(fm + e), h[e],
+                           closure_on(P, d), s0 - 1 + e, dim_n(P, d));
         }
         for (int m = 0; m < 5; ++m) out[m] -= J * (h[1][m] - h[0][m]);
     }

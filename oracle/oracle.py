@@ -35,6 +35,7 @@ class OraParams(C.Structure):
         ("inflow", _dp * 6),
         ("visc_order", C.c_int),
         ("bc_closure", C.c_int),
+        ("char_recon", C.c_int),
     ]
 
 
@@ -87,6 +88,15 @@ def weno5(f, eps=1e-6):
     f = np.ascontiguousarray(f, dtype=np.float64)
     assert f.shape == (5,)
     return lib().ora_weno5(_ptr(f), C.c_double(eps))
+
+
+def eigen_matrices(gamma, u, v, w, c, n):
+    """S (eq. 35) and S^-1 (eq. 34) of PAPER.md:L236-238 for the unit direction n."""
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    S, Si = np.zeros((5, 5)), np.zeros((5, 5))
+    d = C.c_double
+    lib().ora_eigen_matrices(d(gamma), d(u), d(v), d(w), d(c), _ptr(n), _ptr(S), _ptr(Si))
+    return S, Si
 
 
 def weno5_masked(f, keep, nearest, eps=1e-6):
@@ -146,6 +156,7 @@ def params_from_case(case):
     P.inviscid = 1 if case.inviscid else 0
     P.visc_order = int(getattr(case, "visc_order", 6))
     P.bc_closure = int(getattr(case, "bc_closure", 0))
+    P.char_recon = int(getattr(case, "char_recon", 0))
     P.scheme = SCHEMES[case.scheme]
     P.theta1, P.theta2 = case.theta1, case.theta2
     P.weno_eps, P.sw_eps = case.weno_eps, case.sw_eps
