@@ -48,6 +48,12 @@ WORKLOADS = {
     "ramp2048x300x256_hybrid_closure": (lambda: _with(W.ramp(), bc_closure=1),
                                         lambda: _with(W.ramp(nx=512, ny=76, nz=32), bc_closure=1),
                                         "configs[4] with the paper's inviscid boundary scheme (SURVEY 8(f) NEXT #1)"),
+    "ramp2048x300x256_hybrid_char": (lambda: _with(W.ramp(), char_recon=1),
+                                     lambda: _with(W.ramp(nx=512, ny=76, nz=32), char_recon=1),
+                                     "configs[4] with reconstruction in characteristic variables (SURVEY 8(f) NEXT #2)"),
+    "ramp2048x300x256_weno7_char": (lambda: _with(W.ramp(scheme="weno7"), char_recon=1),
+                                    lambda: _with(W.ramp(nx=512, ny=76, nz=32, scheme="weno7"), char_recon=1),
+                                    "configs[4] grid, WENO7 everywhere in characteristic variables (ALU-bound)"),
     "ramp512x76x32_hybrid": (lambda: W.ramp(nx=512, ny=76, nz=32), lambda: W.ramp(nx=512, ny=76, nz=32), "small twin"),
     "ramp1024x152x64_hybrid": (lambda: W.ramp(nx=1024, ny=152, nz=64), lambda: W.ramp(nx=512, ny=76, nz=32),
                                "mid-size twin (ncu captures)"),

@@ -95,6 +95,10 @@ typedef struct {
      * candidates are shielded (the boundary interface itself, for the wave that enters) the boundary node's split
      * flux is taken (DESIGN R-21). */
     int bc_closure;
+    /* 1: flux reconstruction in characteristic variables (section 2.2.2): at every interface the
+     * split fluxes of the stencil are projected with the left eigenvectors S (eq. 35) of the averaged state (eq. 32),
+     * reconstructed component by component and projected back with S^-1 (eq. 34).  0: component-wise (default). */
+    int char_recon;
 } ocfd_params;
 
 /* Bytes of device scratch a context with these parameters needs; 0 if the parameters are invalid.  Pure. */

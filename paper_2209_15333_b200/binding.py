@@ -44,6 +44,7 @@ class OcfdParams(C.Structure):
         ("stream", C.c_void_p),
         ("visc_order", C.c_int),
         ("bc_closure", C.c_int),
+        ("char_recon", C.c_int),
     ]
 
 
@@ -117,6 +118,7 @@ def params_from_case(case):
     P.inviscid = 1 if case.inviscid else 0
     P.visc_order = int(getattr(case, "visc_order", 6))
     P.bc_closure = int(getattr(case, "bc_closure", 0))
+    P.char_recon = int(getattr(case, "char_recon", 0))
     P.scheme = SCHEMES[case.scheme]
     P.theta1, P.theta2 = case.theta1, case.theta2
     P.weno_eps, P.sw_eps = case.weno_eps, case.sw_eps

@@ -23,6 +23,7 @@ bool valid_params(const ocfd_params *p) {
     if (p->scheme < OCFD_UD7 || p->scheme > OCFD_HYBRID) return false;
     if (p->visc_order != 0 && p->visc_order != 6 && p->visc_order != 8) return false;
     if (p->bc_closure != 0 && p->bc_closure != 1) return false;
+    if (p->char_recon != 0 && p->char_recon != 1) return false;
     if (p->scheme == OCFD_HYBRID && (isnan(p->theta1) || isnan(p->theta2))) return false;
     switch (p->grid_kind) {
         case OCFD_GRID_UNIFORM:

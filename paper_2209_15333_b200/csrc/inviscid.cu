@@ -59,11 +59,15 @@ __device__ __forceinline__ void tile_coords(int t, int nts, int nta, int &ts, in
 
 // KIND: grid kind, SCHEME: ocfd_scheme, DIR: 0 x, 1 y, 2 z.  Persistent: CTA b processes tiles b, b + gridDim.x, ...;
 // the boxes of the next tile are in flight while the current one is being processed.
-template <int KIND, int SCHEME, int DIR>
-__global__ void __launch_bounds__(INV_NT, 3)
+// CHAR: reconstruction in characteristic variables (ocfd_params.char_recon).  The walkers then only
+// do the interfaces that take the linear scheme (for a linear scheme the projection cancels); every other interface
+// is done by one thread that projects its 8 stencil rows with the S of the interface, component by component.
+template <int KIND, int SCHEME, int DIR, bool CHAR>
+__global__ void __launch_bounds__(INV_NT, CHAR ? ((SCHEME == OCFD_WENO7 || SCHEME == OCFD_WENO5) ? 1 : 2) : 3)
     k_inviscid(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
                const __grid_constant__ CUtensorMap tm_prim, const __grid_constant__ CUtensorMap tm_th,
-               const __grid_constant__ CUtensorMap tm_out, int ntiles, int nts, int nta) {
+               const __grid_constant__ CUtensorMap tm_out, int ntiles, int nts, int nta, const double *__restrict__ Ug,
+               const double *__restrict__ primg) {
     using G = TileGeom<DIR>;
     constexpr int ACP = G::ACP;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -219,7 +223,8 @@ __global__ void __launch_bounds__(INV_NT, 3)
                     wm[6] = fm[(q - q0 + 6) * ACP];
                     const int flag = SCHEME == OCFD_HYBRID ? (int)((mask >> (2 * (q - q0))) & 3u) : 0;
                     double h = 0.0;
-                    if (q < qlive) {
+                    const bool linear = !near_bnd && (SCHEME == OCFD_UD7 || (SCHEME == OCFD_HYBRID && flag == 0));
+                    if (q < qlive && (!CHAR || linear)) {
                         if (near_bnd)
                             h = recon_pair_closure<SCHEME>(flag, o0 - 1 + q, nd, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6],
                                                            wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
@@ -232,6 +237,58 @@ __global__ void __launch_bounds__(INV_NT, 3)
             }
         }
         __syncthreads();
+
+        if (CHAR) {
+            // ---- phase B': the interfaces the walkers left out, in characteristic variables
+            for (int it2 = tid; it2 < NIF * AC; it2 += INV_NT) {
+                const int q = it2 / AC, a = it2 % AC;
+                const int s = o0 - 1 + q;   // interior index of the interface
+                if (a0 + a >= na || s > nd - 1) continue;
+                const int seg = q / SL;
+                int flag = 0;
+                if (SCHEME == OCFD_HYBRID) {
+                    unsigned mask = 0u;
+#pragma unroll
+                    for (int e = 0; e < 5; ++e) mask |= sFl[(seg * 5 + e) * AC + a];
+                    flag = (int)((mask >> (2 * (q - seg * SL))) & 3u);
+                }
+                const bool near_if = g.closure[DIR] && (s <= 2 || s >= nd - 4);
+                if (!near_if && (SCHEME == OCFD_UD7 || (SCHEME == OCFD_HYBRID && flag == 0))) continue;
+                // averaged conserved state of the two points of the interface (eq. 32) and its direction
+                // n = (alpha_s + alpha_s+1) normalised (DESIGN R-22), from global memory (the staged copies are gone)
+                double rb = 0.0, mx = 0.0, my = 0.0, mz = 0.0, Eb = 0.0, n0 = 0.0, n1 = 0.0, n2 = 0.0;
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int sp = o0 + q + 3 + e, ap = OCFD_NG + a0 + a;
+                    const int ip = DIR == 0 ? sp : ap, jp = DIR == 0 ? ap : DIR == 1 ? sp : OCFD_NG + cross;
+                    const int kp = DIR == 2 ? sp : OCFD_NG + cross;
+                    const long long id = pidx(g, ip, jp, kp);
+                    const double r = __ldg(Ug + id), u = __ldg(primg + P_U * g.np + id), v = __ldg(primg + P_V * g.np + id);
+                    const double w = __ldg(primg + P_W * g.np + id), c = __ldg(primg + P_C * g.np + id);
+                    rb += 0.5 * r; mx += 0.5 * r * u; my += 0.5 * r * v; mz += 0.5 * r * w;
+                    Eb += 0.5 * (r * c * c / (gs.gamma * gs.gm1) + 0.5 * r * (u * u + v * v + w * w));
+                    double k1, k2, k3, sig, Jd;
+                    met_ksJ<KIND, DIR>(g, ip, jp, kp, k1, k2, k3, sig, Jd);
+                    n0 += k1 * sig; n1 += k2 * sig; n2 += k3 * sig;
+                }
+                const double ub = mx / rb, vb = my / rb, wb = mz / rb;
+                const double pb = gs.gm1 * (Eb - 0.5 * rb * (ub * ub + vb * vb + wb * wb));
+                const double cb = sqrt(gs.gamma * pb / rb);
+                const double rn = rsqrt(n0 * n0 + n1 * n1 + n2 * n2);
+                CharFrame F;
+                F.set(gs.gamma, ub, vb, wb, cb, n0 * rn, n1 * rn, n2 * rn);
+                const double *fp = sF + q * ACP + a, *fm = sF + (5 * ROWS + q) * ACP + a;
+                double h[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+                char_component<SCHEME, 0>(F, flag, near_if, s, nd, fp, fm, ROWS * ACP, ACP, gs.weno_eps, h);
+                char_component<SCHEME, 1>(F, flag, near_if, s, nd, fp, fm, ROWS * ACP, ACP, gs.weno_eps, h);
+                char_component<SCHEME, 2>(F, flag, near_if, s, nd, fp, fm, ROWS * ACP, ACP, gs.weno_eps, h);
+                char_component<SCHEME, 3>(F, flag, near_if, s, nd, fp, fm, ROWS * ACP, ACP, gs.weno_eps, h);
+                char_component<SCHEME, 4>(F, flag, near_if, s, nd, fp, fm, ROWS * ACP, ACP, gs.weno_eps, h);
+#pragma unroll
+                for (int m = 0; m < 5; ++m) sH[(m * NIF + q) * ACP + a] = h[m];
+            }
+            __syncthreads();
+        }
 
         // ---- phase C: dU (-)= J (h_{o+1/2} - h_{o-1/2}) into the output tile, then one TMA store / reduce-add
         for (int pt = tid; pt < OUTS * AC; pt += INV_NT) {
@@ -257,13 +314,13 @@ __global__ void __launch_bounds__(INV_NT, 3)
     if (tid == 0) tma::store_wait_all<0>();
 }
 
-template <int KIND, int SCHEME, int DIR>
-ocfd_status launch_dir(ocfd_ctx *c) {
+template <int KIND, int SCHEME, int DIR, bool CHAR>
+ocfd_status launch_dir(ocfd_ctx *c, const double *U) {
     const GridDesc &g = c->g;
     const size_t shm = TileGeom<DIR>::smem_bytes;
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_inviscid<KIND, SCHEME, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_inviscid<KIND, SCHEME, DIR, CHAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess)
             return OCFD_ECUDA;
         attr_set = true;
     }
@@ -276,24 +333,29 @@ ocfd_status launch_dir(ocfd_ctx *c) {
     const int grid = (int)ntiles;
     OCFD_T0(c, K_INV_X + DIR);
     const InvMaps &M = c->inv;
-    k_inviscid<KIND, SCHEME, DIR><<<grid, INV_NT, shm, c->stream>>>(g, c->gas, M.rho[DIR], M.prim[DIR], M.th[DIR],
-                                                                   M.out[DIR], (int)ntiles, nts, nta);
+    k_inviscid<KIND, SCHEME, DIR, CHAR><<<grid, INV_NT, shm, c->stream>>>(g, c->gas, M.rho[DIR], M.prim[DIR], M.th[DIR],
+                                                                         M.out[DIR], (int)ntiles, nts, nta, U, c->prim);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
 
+// plain: the x sweep (y and z go through the marching kernels); characteristic variables: all three sweeps
 template <int KIND, int SCHEME>
-ocfd_status launch_kind_scheme(ocfd_ctx *c) {
-    return launch_dir<KIND, SCHEME, 0>(c);
+ocfd_status launch_kind_scheme(ocfd_ctx *c, const double *U) {
+    if (!c->p.char_recon) return launch_dir<KIND, SCHEME, 0, false>(c, U);
+    ocfd_status st;
+    if ((st = launch_dir<KIND, SCHEME, 0, true>(c, U)) != OCFD_OK) return st;
+    if ((st = launch_dir<KIND, SCHEME, 1, true>(c, U)) != OCFD_OK) return st;
+    return launch_dir<KIND, SCHEME, 2, true>(c, U);
 }
 
 template <int KIND>
-ocfd_status launch_kind(ocfd_ctx *c) {
+ocfd_status launch_kind(ocfd_ctx *c, const double *U) {
     switch (c->p.scheme) {
-        case OCFD_UD7: return launch_kind_scheme<KIND, OCFD_UD7>(c);
-        case OCFD_WENO7: return launch_kind_scheme<KIND, OCFD_WENO7>(c);
-        case OCFD_WENO5: return launch_kind_scheme<KIND, OCFD_WENO5>(c);
-        default: return launch_kind_scheme<KIND, OCFD_HYBRID>(c);
+        case OCFD_UD7: return launch_kind_scheme<KIND, OCFD_UD7>(c, U);
+        case OCFD_WENO7: return launch_kind_scheme<KIND, OCFD_WENO7>(c, U);
+        case OCFD_WENO5: return launch_kind_scheme<KIND, OCFD_WENO5>(c, U);
+        default: return launch_kind_scheme<KIND, OCFD_HYBRID>(c, U);
     }
 }
 
@@ -328,13 +390,14 @@ bool encode_maps(ocfd_ctx *c, const double *U, double *dU) {
 // dU <- -J sum_d (h_{s+1/2} - h_{s-1/2}); the x sweep writes, y and z accumulate (same order as the definition)
 ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU) {
     ocfd_status st;
-    if (c->x_tile) {
+    if (c->x_tile || c->p.char_recon) {
         if (!encode_maps(c, U, dU)) return OCFD_ECUDA;
         switch (c->g.kind) {
-            case OCFD_GRID_UNIFORM: st = launch_kind<OCFD_GRID_UNIFORM>(c); break;
-            case OCFD_GRID_STRETCHED: st = launch_kind<OCFD_GRID_STRETCHED>(c); break;
-            default: st = launch_kind<OCFD_GRID_CURVILINEAR>(c);
+            case OCFD_GRID_UNIFORM: st = launch_kind<OCFD_GRID_UNIFORM>(c, U); break;
+            case OCFD_GRID_STRETCHED: st = launch_kind<OCFD_GRID_STRETCHED>(c, U); break;
+            default: st = launch_kind<OCFD_GRID_CURVILINEAR>(c, U);
         }
+        if (c->p.char_recon) return st;
     } else {
         st = launch_inviscid_march(c, U, dU, 0);
     }

@@ -140,6 +140,82 @@ __device__ __noinline__ double recon_pair_closure(int flag, int s, int n, double
     return hp + hm;
 }
 
+// ------------------------------------------------------------------------------------------ characteristic variables
+// Eigenvector frame of one interface: unit direction n, l by eq. 39, m = n x l (eq. 40), the
+// averaged state u, v, w, c (eq. 32) and the scalars of eq. 36.  Row k of S (eq. 35) and column k of S^-1 (eq. 34)
+// are produced on demand, so that a thread never holds the two 5 x 5 matrices.
+struct CharFrame {
+    double u, v, w, c, V, H, un, ul, um, kap, chi;
+    double n[3], l[3], m[3];
+    __device__ __forceinline__ void set(double gamma, double u_, double v_, double w_, double c_, double n0, double n1,
+                                        double n2) {
+        u = u_; v = v_; w = w_; c = c_;
+        n[0] = n0; n[1] = n1; n[2] = n2;
+        if (fabs(n2) <= fabs(n1)) {
+            const double r = rsqrt(n0 * n0 + n1 * n1);
+            l[0] = -n1 * r; l[1] = n0 * r; l[2] = 0.0;
+        } else {
+            const double r = rsqrt(n0 * n0 + n2 * n2);
+            l[0] = -n2 * r; l[1] = 0.0; l[2] = n0 * r;
+        }
+        m[0] = n[1] * l[2] - n[2] * l[1]; m[1] = n[2] * l[0] - n[0] * l[2]; m[2] = n[0] * l[1] - n[1] * l[0];
+        V = 0.5 * (u * u + v * v + w * w);
+        H = V + c * c / (gamma - 1.0);
+        un = u * n[0] + v * n[1] + w * n[2]; ul = u * l[0] + v * l[1] + w * l[2]; um = u * m[0] + v * m[1] + w * m[2];
+        kap = (gamma - 1.0) / (c * c);
+        chi = 0.5 / c;
+    }
+    // row K of S
+    template <int K>
+    __device__ __forceinline__ void row(double s[5]) const {
+        const double k1 = 0.5 * kap;
+        if (K == 0) { s[0] = 1.0 - kap * V; s[1] = kap * u; s[2] = kap * v; s[3] = kap * w; s[4] = -kap; }
+        if (K == 1) { s[0] = -ul; s[1] = l[0]; s[2] = l[1]; s[3] = l[2]; s[4] = 0.0; }
+        if (K == 2) { s[0] = -um; s[1] = m[0]; s[2] = m[1]; s[3] = m[2]; s[4] = 0.0; }
+        if (K == 3) { s[0] = k1 * V + chi * un; s[1] = -chi * n[0] - k1 * u; s[2] = -chi * n[1] - k1 * v; s[3] = -chi * n[2] - k1 * w; s[4] = k1; }
+        if (K == 4) { s[0] = k1 * V - chi * un; s[1] = chi * n[0] - k1 * u; s[2] = chi * n[1] - k1 * v; s[3] = chi * n[2] - k1 * w; s[4] = k1; }
+    }
+    // column K of S^-1
+    template <int K>
+    __device__ __forceinline__ void col(double r[5]) const {
+        if (K == 0) { r[0] = 1.0; r[1] = u; r[2] = v; r[3] = w; r[4] = V; }
+        if (K == 1) { r[0] = 0.0; r[1] = l[0]; r[2] = l[1]; r[3] = l[2]; r[4] = ul; }
+        if (K == 2) { r[0] = 0.0; r[1] = m[0]; r[2] = m[1]; r[3] = m[2]; r[4] = um; }
+        if (K == 3) { r[0] = 1.0; r[1] = u - c * n[0]; r[2] = v - c * n[1]; r[3] = w - c * n[2]; r[4] = H - c * un; }
+        if (K == 4) { r[0] = 1.0; r[1] = u + c * n[0]; r[2] = v + c * n[1]; r[3] = w + c * n[2]; r[4] = H + c * un; }
+    }
+};
+
+// One characteristic component K of one interface (eq. 31): project the split fluxes of the 8 stencil rows with row K
+// of S (f+ of rows 0..6, f- of rows 1..7, read from shared memory: fp/fm point at row 0 of component 0, `cs` =
+// component stride, `rs` = row stride), reconstruct, and add column K of S^-1 times the result to h[5].
+template <int SCHEME, int K>
+__device__ __forceinline__ void char_component(const CharFrame &F, int flag, bool closure, int s, int n,
+                                               const double *fp, const double *fm, int cs, int rs, double eps,
+                                               double h[5]) {
+    double sk[5], wp[7], wm[7];
+    F.row<K>(sk);
+#pragma unroll
+    for (int r = 0; r < 7; ++r) {
+        double a = 0.0, b = 0.0;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+            a = fma(sk[q], fp[q * cs + r * rs], a);
+            b = fma(sk[q], fm[q * cs + (r + 1) * rs], b);
+        }
+        wp[r] = a;
+        wm[r] = b;
+    }
+    const double hw = closure ? recon_pair_closure<SCHEME>(flag, s, n, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6],
+                                                           wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], eps)
+                              : recon<SCHEME>(flag, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6], eps) +
+                                    recon<SCHEME>(flag, wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], eps);
+    double rk[5];
+    F.col<K>(rk);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) h[q] = fma(rk[q], hw, h[q]);
+}
+
 // ------------------------------------------------------------------------------------------ Steger-Warming
 // Split fluxes of direction DIR at one point, written to sF[c*cs], c = 0..9 (eq. 19-29 with the
 // readings R-4, R-5, R-7).  k = alpha/|alpha| (unit), sigma = |alpha|, alpha = (d_x,d_y,d_z)/J.

@@ -228,6 +228,39 @@ def test_twenty_steps_paper_boundary_scheme(B, Oracle):
     assert np.isfinite(got).all()
 
 
+@pytest.mark.parametrize("which", ["wavy-ud7", "wavy-weno7", "wavy-weno5", "stretched-hybrid", "uniform-weno7",
+                                   "shocked", "plate", "ramp3level", "box-closure"])
+def test_rhs_parity_characteristic_reconstruction(B, Oracle, which):
+    """char_recon = 1 (PAPER.md:L212-263, SURVEY 8(f) NEXT #2): all three sweeps in characteristic variables."""
+    if which == "plate":
+        case = W.flat_plate(nx=72, ny=44, nz=24)
+    elif which == "ramp3level":
+        case = W.ramp(nx=64, ny=44, nz=24, nmodes=12, theta2=0.1)
+    elif which == "shocked":
+        case = W.shocked_periodic(44, theta1=0.02, theta2=0.1)
+    elif which == "box-closure":
+        case = W.smooth_periodic(70, 45, 23, grid="wavy", scheme="weno7", Re=150.0, seed=6)
+        case.bc = ["outflow"] * 6
+        case.bc_closure = 1
+    else:
+        grid, scheme = which.split("-")
+        case = W.smooth_periodic(70, 45, 23, grid=grid, scheme=scheme, Re=150.0, seed=8)
+    case.char_recon = 1
+    got, ref, U = run_rhs_both(B, Oracle, case)
+    floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
+    err = rel_linf(got, ref, U, floor)
+    print(which, "rel Linf per component", err)
+    assert err.max() <= TOL_RHS
+
+
+def test_ten_steps_characteristic_reconstruction(B, Oracle):
+    case = W.tgv(24, nsteps=10)
+    case.char_recon = 1
+    err, _, _ = step_both(B, Oracle, case, 10, check_every=5)
+    print("TGV 24^3, WENO7 in characteristic variables, 10 steps: rel Linf", err)
+    assert err <= TOL_100
+
+
 def test_ten_steps_eighth_order_viscous_scheme(B, Oracle):
     case = W.tgv(24, nsteps=10)
     case.visc_order = 8
