@@ -253,6 +253,34 @@ def test_rhs_parity_characteristic_reconstruction(B, Oracle, which):
     assert err.max() <= TOL_RHS
 
 
+@pytest.mark.parametrize("dims", [(8, 8, 8), (10, 9, 8), (34, 8, 33), (8, 37, 9)])
+@pytest.mark.parametrize("scheme", ["hybrid", "weno7"])
+def test_rhs_parity_smallest_and_ragged_grids(B, Oracle, dims, scheme):
+    """Edge sizes: the minimum the library accepts (8 points per axis: the march is four chunks, the x tile one
+    ragged tile, the viscous tiles mostly empty), and extents one or two past a tile / chunk boundary."""
+    nx, ny, nz = dims
+    for grid in ("uniform", "wavy"):
+        case = W.smooth_periodic(nx, ny, nz, grid=grid, scheme=scheme, Re=120.0, seed=nx + ny + nz)
+        got, ref, U = run_rhs_both(B, Oracle, case)
+        assert rel_linf(got, ref, U).max() <= TOL_RHS, (dims, grid)
+
+
+def test_invalid_parameters_are_refused_without_touching_buffers(B):
+    """Argument errors come back as status codes (never exceptions from the library), synchronously."""
+    case = W.smooth_periodic(8, 8, 8)
+    for field, bad in (("nx", 9), ("nx", 6), ("visc_order", 7), ("bc_closure", 2), ("char_recon", -1)):
+        broken = W.smooth_periodic(8, 8, 8)
+        if field == "nx":
+            broken.nx = bad          # odd, or below the minimum
+        else:
+            setattr(broken, field, bad)
+        with pytest.raises(Exception) as e:
+            B.Solver(broken)
+        assert "invalid" in str(e.value).lower() or "workspace" in str(e.value).lower() or "shape" in str(e.value).lower()
+    s = B.Solver(case)               # and a valid one still works afterwards
+    s.close()
+
+
 def test_ten_steps_characteristic_reconstruction(B, Oracle):
     case = W.tgv(24, nsteps=10)
     case.char_recon = 1
