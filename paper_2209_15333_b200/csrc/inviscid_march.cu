@@ -249,6 +249,23 @@ __global__ void __launch_bounds__(MNT, 4)
                 else so[e * MAC] = -Jw[e] * (h - hprev);
                 hprev = h;
             }
+        } else if (near_bnd) {
+            // chunks next to an aperiodic boundary under the paper's boundary scheme: every interface is tested (a
+            // branch of its own, so that the out-of-line call does not weigh on the general path below)
+#pragma unroll
+            for (int e = 0; e < MR; ++e) {
+                const int k = 4 * PH + e;
+                Wp[k & 7] = nP[e];
+                Wm[k & 7] = nM[e];
+                const int flag = SCHEME == OCFD_HYBRID ? (int)((cur >> (2 * e)) & 3u) : 0;
+                const double h = recon_pair_closure<SCHEME>(
+                    flag, r0 + e - 2 * OCFD_NG, nd, Wp[(k + 1) & 7], Wp[(k + 2) & 7], Wp[(k + 3) & 7], Wp[(k + 4) & 7],
+                    Wp[(k + 5) & 7], Wp[(k + 6) & 7], Wp[(k + 7) & 7], Wm[k & 7], Wm[(k + 7) & 7], Wm[(k + 6) & 7],
+                    Wm[(k + 5) & 7], Wm[(k + 4) & 7], Wm[(k + 3) & 7], Wm[(k + 2) & 7], gs.weno_eps);
+                if (DIR == 0) out[e] = -Jw[e] * (h - hprev);
+                else so[e * MAC] = -Jw[e] * (h - hprev);
+                hprev = h;
+            }
         } else {
 #pragma unroll
             for (int e = 0; e < MR; ++e) {
@@ -256,16 +273,10 @@ __global__ void __launch_bounds__(MNT, 4)
                 Wp[k & 7] = nP[e];
                 Wm[k & 7] = nM[e];
                 const int flag = SCHEME == OCFD_HYBRID ? (int)((cur >> (2 * e)) & 3u) : 0;
-                const double h =
-                    near_bnd ? recon_pair_closure<SCHEME>(flag, r0 + e - 2 * OCFD_NG, nd, Wp[(k + 1) & 7], Wp[(k + 2) & 7],
-                                                          Wp[(k + 3) & 7], Wp[(k + 4) & 7], Wp[(k + 5) & 7], Wp[(k + 6) & 7],
-                                                          Wp[(k + 7) & 7], Wm[k & 7], Wm[(k + 7) & 7], Wm[(k + 6) & 7],
-                                                          Wm[(k + 5) & 7], Wm[(k + 4) & 7], Wm[(k + 3) & 7], Wm[(k + 2) & 7],
-                                                          gs.weno_eps)
-                             : recon_pair<SCHEME>(flag, Wp[(k + 1) & 7], Wp[(k + 2) & 7], Wp[(k + 3) & 7], Wp[(k + 4) & 7],
-                                                  Wp[(k + 5) & 7], Wp[(k + 6) & 7], Wp[(k + 7) & 7], Wm[k & 7],
-                                                  Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
-                                                  Wm[(k + 3) & 7], Wm[(k + 2) & 7], gs.weno_eps);
+                const double h = recon_pair<SCHEME>(flag, Wp[(k + 1) & 7], Wp[(k + 2) & 7], Wp[(k + 3) & 7], Wp[(k + 4) & 7],
+                                                    Wp[(k + 5) & 7], Wp[(k + 6) & 7], Wp[(k + 7) & 7], Wm[k & 7],
+                                                    Wm[(k + 7) & 7], Wm[(k + 6) & 7], Wm[(k + 5) & 7], Wm[(k + 4) & 7],
+                                                    Wm[(k + 3) & 7], Wm[(k + 2) & 7], gs.weno_eps);
                 if (DIR == 0) out[e] = -Jw[e] * (h - hprev);
                 else so[e * MAC] = -Jw[e] * (h - hprev);
                 hprev = h;
