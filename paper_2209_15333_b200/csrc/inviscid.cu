@@ -206,6 +206,25 @@ __global__ void __launch_bounds__(INV_NT, CHAR ? ((SCHEME == OCFD_WENO7 || SCHEM
                                      ud7(wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0]);
                     if (q0 + i < NIF) sH[(m * NIF + q0 + i) * ACP + a] = h;
                 }
+            } else if (near_bnd) {
+                // segments next to an aperiodic boundary under the paper's boundary scheme: every interface is tested
+                // (a loop of its own, so that the out-of-line call does not weigh on the general loop below)
+#pragma unroll 1
+                for (int q = q0; q < qend; ++q) {
+#pragma unroll
+                    for (int e = 0; e < 6; ++e) {
+                        wp[e] = wp[e + 1];
+                        wm[e] = wm[e + 1];
+                    }
+                    wp[6] = fp[(q - q0 + 6) * ACP];
+                    wm[6] = fm[(q - q0 + 6) * ACP];
+                    const int flag = SCHEME == OCFD_HYBRID ? (int)((mask >> (2 * (q - q0))) & 3u) : 0;
+                    double h = 0.0;
+                    if (q < qlive && !CHAR)
+                        h = recon_pair_closure<SCHEME>(flag, o0 - 1 + q, nd, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6],
+                                                       wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
+                    sH[(m * NIF + q) * ACP + a] = h;
+                }
             } else {
 #pragma unroll 1
                 for (int q = q0; q < qend; ++q) {
@@ -218,15 +237,10 @@ __global__ void __launch_bounds__(INV_NT, CHAR ? ((SCHEME == OCFD_WENO7 || SCHEM
                     wm[6] = fm[(q - q0 + 6) * ACP];
                     const int flag = SCHEME == OCFD_HYBRID ? (int)((mask >> (2 * (q - q0))) & 3u) : 0;
                     double h = 0.0;
-                    const bool linear = !near_bnd && (SCHEME == OCFD_UD7 || (SCHEME == OCFD_HYBRID && flag == 0));
-                    if (q < qlive && (!CHAR || linear)) {
-                        if (near_bnd)
-                            h = recon_pair_closure<SCHEME>(flag, o0 - 1 + q, nd, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6],
-                                                           wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
-                        else
-                            h = recon<SCHEME>(flag, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6], gs.weno_eps) +
-                                recon<SCHEME>(flag, wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
-                    }
+                    const bool linear = SCHEME == OCFD_UD7 || (SCHEME == OCFD_HYBRID && flag == 0);
+                    if (q < qlive && (!CHAR || linear))
+                        h = recon<SCHEME>(flag, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6], gs.weno_eps) +
+                            recon<SCHEME>(flag, wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
                     sH[(m * NIF + q) * ACP + a] = h;
                 }
             }
