@@ -265,6 +265,24 @@ def test_rhs_parity_smallest_and_ragged_grids(B, Oracle, dims, scheme):
         assert rel_linf(got, ref, U).max() <= TOL_RHS, (dims, grid)
 
 
+def test_results_are_bitwise_reproducible(B):
+    """One add per output element and kernel (TMA reduce-add for y and z, in stream order): no atomics race, so two
+    evaluations of the same state agree bit for bit (the paper's design accumulates with atomicAdd from several
+    streams, and does not have this property)."""
+    case = W.ramp(nx=64, ny=44, nz=24, nmodes=12)
+    s = B.Solver(case)
+    U = s.to_device(case.U0.copy())
+    s.fill_ghosts(U)
+    a = s.rhs(U).clone()
+    b = s.rhs(U).clone()
+    assert bool((a == b).all())
+    U2 = U.clone()
+    s.rk3_step(U, 1e-4)
+    s.rk3_step(U2, 1e-4)
+    assert bool((U == U2).all())
+    s.close()
+
+
 def test_invalid_parameters_are_refused_without_touching_buffers(B):
     """Argument errors come back as status codes (never exceptions from the library), synchronously."""
     case = W.smooth_periodic(8, 8, 8)
