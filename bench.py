@@ -269,6 +269,11 @@ def run_ours(args):
     per_kernel = s.timing_read()
     s.timing(False)
     finite = bool(torch.isfinite(U).all().item())
+    flag_hist_end = None
+    if case.scheme == "hybrid":     # after the warm-up and timed steps (outside the timed region)
+        _, fl = s.debug_sensor(U)
+        flag_hist_end = torch.bincount(fl[fl < 3].flatten().to(torch.int64), minlength=3).cpu().numpy()
+        del fl
     ms_all = max_over_ranks(ms, world, s.device)
     value = whole_job_value(ms * 1e-3, case.npoints, args.steps, world, s.device)
 
@@ -341,6 +346,7 @@ def run_ours(args):
                    "parallelism": "single GPU" if world == 1 else f"{world} independent replicas",
                    "cache": "inputs larger than L2 (state 5 fields x %.0f MB)" % (np.prod(case.padded_shape) * 8 / 1e6),
                    "hybrid_flag_hist_ud7_weno7_weno5": None if flag_hist is None else [int(v) for v in flag_hist],
+                   "hybrid_flag_hist_after_steps": None if flag_hist_end is None else [int(v) for v in flag_hist_end],
                    "input_generation_s": t_gen, "finite": finite},
         "clocks": clk.summary(),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
