@@ -58,7 +58,7 @@ __device__ __forceinline__ void tile_coords(int &ts, int &ta, int &cross) {
 // do the interfaces that take the linear scheme (for a linear scheme the projection cancels); every other interface
 // is done by one thread that projects its 8 stencil rows with the S of the interface, component by component.
 template <int KIND, int SCHEME, int DIR, bool CHAR>
-__global__ void __launch_bounds__(INV_NT, CHAR ? ((SCHEME == OCFD_WENO7 || SCHEME == OCFD_WENO5) ? 1 : 2) : 3)
+__global__ void __launch_bounds__(INV_NT, CHAR ? 2 : 3)
     k_inviscid(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
                const __grid_constant__ CUtensorMap tm_prim, const __grid_constant__ CUtensorMap tm_th,
                const __grid_constant__ CUtensorMap tm_out, const double *__restrict__ Ug,

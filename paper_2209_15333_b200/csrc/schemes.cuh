@@ -190,7 +190,7 @@ struct CharFrame {
 // of S (f+ of rows 0..6, f- of rows 1..7, read from shared memory: fp/fm point at row 0 of component 0, `cs` =
 // component stride, `rs` = row stride), reconstruct, and add column K of S^-1 times the result to h[5].
 template <int SCHEME, int K>
-__device__ __forceinline__ void char_component(const CharFrame &F, int flag, bool closure, int s, int n,
+__device__ __noinline__ void char_component(const CharFrame &F, int flag, bool closure, int s, int n,
                                                const double *fp, const double *fm, int cs, int rs, double eps,
                                                double h[5]) {
     double sk[5], wp[7], wm[7];
