@@ -54,6 +54,8 @@ WORKLOADS = {
     "ramp2048x300x256_weno7_char": (lambda: _with(W.ramp(scheme="weno7"), char_recon=1),
                                     lambda: _with(W.ramp(nx=512, ny=76, nz=32, scheme="weno7"), char_recon=1),
                                     "configs[4] grid, WENO7 everywhere in characteristic variables (ALU-bound)"),
+    "ramp2048x300x256_ud7": (lambda: W.ramp(scheme="ud7"), lambda: W.ramp(nx=512, ny=76, nz=32, scheme="ud7"),
+                             "configs[4] grid with the linear 7th-order scheme everywhere (no sensor, no flags)"),
     "ramp512x76x32_hybrid": (lambda: W.ramp(nx=512, ny=76, nz=32), lambda: W.ramp(nx=512, ny=76, nz=32), "small twin"),
     "ramp1024x152x64_hybrid": (lambda: W.ramp(nx=1024, ny=152, nz=64), lambda: W.ramp(nx=512, ny=76, nz=32),
                                "mid-size twin (ncu captures)"),
