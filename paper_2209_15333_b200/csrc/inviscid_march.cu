@@ -83,7 +83,7 @@ __device__ __forceinline__ double recon_pair(int flag, double p0, double p1, dou
 // that both the point-wise phase and the walkers are free of bank conflicts, and the output tile is written as two
 // 16-byte stores per walker and leaves by a TMA store (the x sweep writes dU, y and z accumulate).
 template <int KIND, int SCHEME, int DIR>
-__global__ void __launch_bounds__(MNT, 4)
+__global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
     k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
                      const __grid_constant__ CUtensorMap tm_prim, const __grid_constant__ CUtensorMap tm_th,
                      const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_met,
