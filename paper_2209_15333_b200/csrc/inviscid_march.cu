@@ -82,6 +82,9 @@ __device__ __forceinline__ double recon_pair(int flag, double p0, double p1, dou
 // shared arrays keep the box order (x fastest), the split fluxes are stored with an XOR swizzle of the pencil index so
 // that both the point-wise phase and the walkers are free of bank conflicts, and the output tile is written as two
 // 16-byte stores per walker and leaves by a TMA store (the x sweep writes dU, y and z accumulate).
+// Occupancy: 4 CTAs per SM (96 registers) except for the hybrid scheme, whose three code paths need 128 registers to keep
+// the unrolled linear path free of spills (measured: 3.8 ms against 4.5 ms per sweep on config 5; the WENO7 kernels
+// gain nothing from the extra registers).
 template <int KIND, int SCHEME, int DIR>
 __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
     k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
