@@ -103,8 +103,13 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->stream = (cudaStream_t)p->stream;
     c->nsm = nsm;
     {
+        // x sweep: the marching kernel for the linear and hybrid schemes (4.4 against 4.75 ms on config 5), the tile kernel
+        // for WENO everywhere (ALU-bound; the march has too few CTAs on grids with a short y axis).  OCFD_X_SWEEP = tile
+        // or march overrides (A/B runs, profiles/r01_c_x_sweep_ab.md).
         const char *e = getenv("OCFD_X_SWEEP");
-        c->x_tile = !(e && !strcmp(e, "march"));   // measured: the tile kernel is 15 % faster (profiles/)
+        c->x_tile = p->scheme == OCFD_WENO7 || p->scheme == OCFD_WENO5;
+        if (e && !strcmp(e, "tile")) c->x_tile = 1;
+        if (e && !strcmp(e, "march")) c->x_tile = 0;
     }
     c->visc_order = p->visc_order == 8 ? 8 : 6;
     GridDesc &g = c->g;

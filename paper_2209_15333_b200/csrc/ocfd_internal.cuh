@@ -79,7 +79,7 @@ struct ocfd_ctx {
     GasDesc gas;
     cudaStream_t stream;
     int visc_order;  // 6 or 8 (ocfd_params.visc_order, 0 -> 6)
-    int x_tile;      // 1 (default): x sweep by the tile kernel of inviscid.cu; 0 (environment OCFD_X_SWEEP=march): marching kernel
+    int x_tile;      // x sweep by the tile kernel of inviscid.cu (1: default for WENO7 / WENO5) or the marching kernel (0: UD7, hybrid)
     int nsm;         // SM count of the device (persistent kernels launch a multiple of it)
     // workspace carve-up (device pointers)
     double *prim;    // [6][np]: T u v w c p
