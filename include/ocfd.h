@@ -104,7 +104,11 @@ typedef struct {
 /* Bytes of device scratch a context with these parameters needs; 0 if the parameters are invalid.  Pure. */
 size_t ocfd_workspace_bytes(const ocfd_params *p);
 
-/* Validate, copy the parameters, carve the workspace.  No field memory is allocated. */
+/* Validate, copy the parameters, carve the workspace, build the derived metric tables (one small launch on the stream).
+ * No field memory is allocated.  Errors: OCFD_EINVAL (parameters), OCFD_EWORKSPACE, OCFD_EUNSUPPORTED (not an sm_100
+ * device), OCFD_ECUDA.  Tuning knob, read here once: environment variable OCFD_X_SWEEP = "tile" | "march" forces the
+ * kernel of the x sweep (default: marching kernel for UD7 / HYBRID, tile kernel for WENO7 / WENO5); results are the
+ * same to round-off. */
 ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p);
 ocfd_status ocfd_destroy(ocfd_ctx *ctx);
 
