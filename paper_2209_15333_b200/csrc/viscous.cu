@@ -94,7 +94,8 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     auto issue = [&](int plane) {  // plane k (interior index) -> stage (k - k0) % NST
         const int s = (plane - k0) % VF_NST;
         tma::mbar_expect_tx(&bars[s], VF_STAGE * 8);
-        tma::load4(ring + s * VF_STAGE, &tm_prim, &bars[s], i0, j0 + OCFD_NG - H, plane + OCFD_NG, 0);
+        tma::load4_hint(ring + s * VF_STAGE, &tm_prim, &bars[s], i0, j0 + OCFD_NG - H, plane + OCFD_NG, 0,
+                        tma::policy_evict_last());   // the halo of this box is a neighbouring tile's interior
     };
     if (tid == 0) {
         for (int s = 0; s < VF_NST; ++s) tma::mbar_init(&bars[s], 1);
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
                 const double f0 = dx * txx + dy * txy + dz * txz, f1 = dx * txy + dy * tyy + dz * tyz;
                 const double f2 = dx * txz + dy * tyz + dz * tzz, f3 = dx * thx + dy * thy + dz * thz;
                 double *F = Fv + (4 * d) * g.np;
-                F[id] = f0; F[g.np + id] = f1; F[2 * g.np + id] = f2; F[3 * g.np + id] = f3;
+                __stcs(F + id, f0); __stcs(F + g.np + id, f1); __stcs(F + 2 * g.np + id, f2); __stcs(F + 3 * g.np + id, f3);
                 if (g.periodic[d]) {  // images beyond the faces of this direction's own axis
                     long long im = -1;
                     if (c[d] < H) im = id + n[d] * st[d];
@@ -234,6 +235,7 @@ __global__ void __launch_bounds__(VNT, 1)
         double *b = ring + s * VD_STAGE;
         const int xp = i0 + OCFD_NG, yp = j0 + OCFD_NG, kp = k + OCFD_NG;
         tma::mbar_expect_tx(&bars[s], BYTES);
+        // (plain loads: L2 eviction hints on these boxes were measured and cost 10 %, profiles/r01_c)
         tma::load4(b, &tm_F, &bars[s], xp - 4, yp, kp, 0);
         tma::load4(b + VD_F, &tm_G, &bars[s], xp, yp - HH, kp, 4);
         tma::load4(b + VD_F + VD_G, &tm_H, &bars[s], xp, yp, kp + HH, 8);
@@ -291,12 +293,12 @@ __global__ void __launch_bounds__(VNT, 1)
                     const long long q = m * g.np + id;
                     const double u = sU[m * TY * TX + ctr];
                     if (RK == 1) {
-                        Un[q] = u;
-                        U[q] = u + dt * acc[m];
+                        __stcs(Un + q, u);
+                        __stcs(U + q, u + dt * acc[m]);
                     } else if (RK == 2) {
-                        U[q] = 0.75 * sUn[m * TY * TX + ctr] + 0.25 * (u + dt * acc[m]);
+                        __stcs(U + q, 0.75 * sUn[m * TY * TX + ctr] + 0.25 * (u + dt * acc[m]));
                     } else {
-                        U[q] = (1.0 / 3.0) * sUn[m * TY * TX + ctr] + (2.0 / 3.0) * (u + dt * acc[m]);
+                        __stcs(U + q, (1.0 / 3.0) * sUn[m * TY * TX + ctr] + (2.0 / 3.0) * (u + dt * acc[m]));
                     }
                 }
             }
