@@ -37,12 +37,12 @@ __global__ void __launch_bounds__(256) k_prim(long long np, GasDesc gs, const do
             T.x = gs.gM2 * p.x / q[e][0].x; T.y = gs.gM2 * p.y / q[e][0].y;
             c.x = sqrt(T.x) * gs.invMa; c.y = sqrt(T.y) * gs.invMa;
             const long long o = id + e * stride;
-            __stcs(P2 + P_U * npair + o, u);
-            __stcs(P2 + P_V * npair + o, v);
-            __stcs(P2 + P_W * npair + o, w);
-            __stcs(P2 + P_T * npair + o, T);
-            __stcs(P2 + P_C * npair + o, c);
-            __stcs(P2 + P_P * npair + o, p);
+            P2[P_U * npair + o] = u;
+            P2[P_V * npair + o] = v;
+            P2[P_W * npair + o] = w;
+            P2[P_T * npair + o] = T;
+            P2[P_C * npair + o] = c;
+            P2[P_P * npair + o] = p;
         }
     }
 }
