@@ -265,6 +265,39 @@ def test_rhs_parity_smallest_and_ragged_grids(B, Oracle, dims, scheme):
         assert rel_linf(got, ref, U).max() <= TOL_RHS, (dims, grid)
 
 
+def test_host_buffer_entry_point_equals_the_device_path_and_the_oracle(B, Oracle):
+    """ocfd_rk3_steps_host (H2D, n steps, D2H in one call: the end-to-end number of bench.py goes through it)."""
+    import torch
+    case = W.ramp(nx=64, ny=40, nz=16, nmodes=12)
+    o = Oracle(case)
+    U = o.fill_ghosts(case.U0.copy())
+    dt = case.cfl / o.max_wavespeed(U)
+    s = B.Solver(case)
+    Ud = s.to_device(U)
+    Uh = torch.from_numpy(U.copy()).pin_memory()
+    scratch = torch.empty_like(Ud)
+    s.rk3_steps_host(Uh, scratch, dt, 2)
+    for _ in range(2):
+        s.rk3_step(Ud, dt)
+        o.rk3_step(U, dt)
+    assert bool((Uh == Ud.cpu()).all())
+    got = Uh.numpy()
+    assert max(np.abs(got[m] - U[m]).max() / np.abs(U[m]).max() for m in range(5)) <= 1e-11
+    s.close()
+
+
+@pytest.mark.parametrize("which", ["plate", "ramp", "wavy"])
+def test_max_wavespeed_matches_the_oracle(B, Oracle, which):
+    case = (W.flat_plate(nx=72, ny=44, nz=24) if which == "plate" else W.ramp(nx=64, ny=44, nz=24, nmodes=12)
+            if which == "ramp" else W.smooth_periodic(70, 45, 23, grid="wavy"))
+    o = Oracle(case)
+    U = o.fill_ghosts(case.U0.copy())
+    s = B.Solver(case)
+    lam = s.max_wavespeed(s.to_device(U))
+    s.close()
+    assert lam == pytest.approx(o.max_wavespeed(U), rel=1e-13)
+
+
 def test_results_are_bitwise_reproducible(B):
     """One add per output element and kernel (TMA reduce-add for y and z, in stream order): no atomics race, so two
     evaluations of the same state agree bit for bit (the paper's design accumulates with atomicAdd from several
