@@ -107,7 +107,9 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
         // for WENO everywhere (ALU-bound; the march has too few CTAs on grids with a short y axis).  OCFD_X_SWEEP = tile
         // or march overrides (A/B runs, profiles/r01_c_x_sweep_ab.md).
         const char *e = getenv("OCFD_X_SWEEP");
-        c->x_tile = p->scheme == OCFD_WENO7 || p->scheme == OCFD_WENO5;
+        // ... and for grids whose y-z cross-section gives the march fewer than two waves of CTAs (32 y-lines each)
+        c->x_tile = p->scheme == OCFD_WENO7 || p->scheme == OCFD_WENO5 ||
+                    (long long)((p->ny + 31) / 32) * p->nz < 2ll * 3 * nsm;
         if (e && !strcmp(e, "tile")) c->x_tile = 1;
         if (e && !strcmp(e, "march")) c->x_tile = 0;
     }
