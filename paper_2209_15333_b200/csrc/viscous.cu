@@ -13,6 +13,8 @@
 #include "schemes.cuh"
 #include "tma.cuh"
 
+#include <stdlib.h>
+
 namespace {
 
 constexpr int TX = 32, TY = 8, VNT = TX * TY;  // own points of a tile = threads
@@ -308,11 +310,20 @@ __global__ void __launch_bounds__(VNT, 1)
     }
 }
 
-int pick_zchunk(const GridDesc &g) {
-    // enough blocks to fill 148 SMs a few times over, chunks long enough that the prologue planes stay cheap
+int pick_zchunk(const GridDesc &g, int pass) {
+    // enough blocks to fill 148 SMs a few times over ...
     const long long tiles = (long long)((g.nx + TX - 1) / TX) * ((g.ny + TY - 1) / TY);
     int zc = g.nz;
     while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < 148 * 8) zc = (zc + 1) / 2;
+    // ... and short enough that tiles which share a halo stay close in z: CTAs drift apart while they march, and a
+    // halo plane the neighbour read long ago has left the L2.  Measured on config 5 (profiles/r01_c): chunks of 64
+    // planes for pass 1 (4.94 -> 4.73 ms) and 32 for pass 2 (7.99 -> 7.02 ms); the prologue planes of a chunk come from L2.
+    const int cap = pass == 1 ? 64 : 32;
+    if (zc > cap) zc = cap;
+    if (const char *e = getenv(pass == 1 ? "OCFD_ZCHUNK_F" : "OCFD_ZCHUNK_D")) {   // tuning knob for A/B runs
+        const int v = atoi(e);
+        if (v >= 8) zc = v < g.nz ? v : g.nz;
+    }
     return zc;
 }
 
@@ -368,18 +379,19 @@ ocfd_status launch_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_st
             return OCFD_ECUDA;
         attr_set = true;
     }
-    const int zc = pick_zchunk(g);
+    const int zc = pick_zchunk(g, 1), zcd = pick_zchunk(g, 2);
     dim3 blk(TX, TY, 1), grd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zc - 1) / zc);
+    dim3 grdd(grd.x, grd.y, (g.nz + zcd - 1) / zcd);
     OCFD_T0(c, K_VISC_FLUX);
     k_viscous_flux<KIND, ORDER><<<grd, blk, VF<ORDER>::SMEM, c->stream>>>(g, c->gas, c->visc.prim, c->prim, c->Fv, zc);
     OCFD_CHECK_LAUNCH(c);
     OCFD_T0(c, K_VISC_DIV);
     ocfd_status st;
     switch (rk_stage) {
-        case 0: st = launch_div<KIND, 1, ORDER>(c, grd, blk, dU, U, dt, zc); break;
-        case 1: st = launch_div<KIND, 2, ORDER>(c, grd, blk, dU, U, dt, zc); break;
-        case 2: st = launch_div<KIND, 3, ORDER>(c, grd, blk, dU, U, dt, zc); break;
-        default: st = launch_div<KIND, 0, ORDER>(c, grd, blk, dU, nullptr, 0.0, zc);
+        case 0: st = launch_div<KIND, 1, ORDER>(c, grdd, blk, dU, U, dt, zcd); break;
+        case 1: st = launch_div<KIND, 2, ORDER>(c, grdd, blk, dU, U, dt, zcd); break;
+        case 2: st = launch_div<KIND, 3, ORDER>(c, grdd, blk, dU, U, dt, zcd); break;
+        default: st = launch_div<KIND, 0, ORDER>(c, grdd, blk, dU, nullptr, 0.0, zcd);
     }
     if (st != OCFD_OK) return st;
     OCFD_CHECK_LAUNCH(c);
