@@ -28,6 +28,8 @@ extern "C" {
 
 typedef struct ocfd_ctx ocfd_ctx; /* opaque; owns no device memory */
 
+#define OCFD_MAX_EXTENT 65527 /* largest interior extent per axis (an extent + 8 is a CUDA grid dimension) */
+
 typedef enum {
     OCFD_OK = 0,
     OCFD_EINVAL = -1,       /* bad argument (null pointer, bad size, inconsistent boundary pairing ...) */
@@ -51,7 +53,8 @@ typedef enum {
 } ocfd_bc;
 
 typedef struct {
-    int nx, ny, nz;   /* interior dimensions, each >= 8 */
+    int nx, ny, nz;   /* interior dimensions, each >= 8 and <= OCFD_MAX_EXTENT; nx must be even (rows of the padded
+                         fields must stay 16-byte aligned for the TMA tensor maps); anything else is OCFD_EINVAL */
     int ng;           /* ghost layers; must be 4 */
     ocfd_grid_kind grid_kind;
     /* Metric data (eq. 3-4), device pointers, caller-owned, must outlive the context.
@@ -71,7 +74,8 @@ typedef struct {
     double gamma, Ma, Re, Pr, T_ref, T_suth;
     int inviscid;            /* 1: skip the viscous terms (rows a6, a7) */
     ocfd_scheme scheme;
-    double theta1, theta2;   /* hybrid thresholds (0.02, 0.1); theta2 = +inf gives two levels */
+    double theta1, theta2;   /* hybrid thresholds (0.02, 0.1), theta1 <= theta2; theta2 = +inf gives two
+                                levels */
     double weno_eps;         /* epsilon of the WENO weights, applied to the J^-1-scaled split flux (DESIGN R-10) */
     double sw_eps;           /* 0: eigenvalue split exactly as eq. 29; > 0: (lambda +- sqrt(lambda^2+eps^2))/2 */
     ocfd_bc bc[6];           /* x-, x+, y-, y+, z-, z+; PERIODIC must be set on both faces of an axis */
@@ -106,9 +110,7 @@ size_t ocfd_workspace_bytes(const ocfd_params *p);
 
 /* Validate, copy the parameters, carve the workspace, build the derived metric tables (one small launch on the stream).
  * No field memory is allocated.  Errors: OCFD_EINVAL (parameters), OCFD_EWORKSPACE, OCFD_EUNSUPPORTED (not an sm_100
- * device), OCFD_ECUDA.  Tuning knob, read here once: environment variable OCFD_X_SWEEP = "tile" | "march" forces the
- * kernel of the x sweep (default: marching kernel for UD7 / HYBRID, tile kernel for WENO7 / WENO5); results are the
- * same to round-off. */
+ * device), OCFD_ECUDA.  The library reads no environment variable and keeps no state outside its contexts. */
 ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p);
 ocfd_status ocfd_destroy(ocfd_ctx *ctx);
 
@@ -137,6 +139,11 @@ ocfd_status ocfd_max_wavespeed(ocfd_ctx *ctx, const double *U, double *host_out)
  * flag_xyz[d][point s] is the scheme of interface s+1/2 along direction d, s = -1 .. n-1.  Either output
  * may be NULL.  Device pointers. */
 ocfd_status ocfd_debug_sensor(ocfd_ctx *ctx, const double *U, double *theta, unsigned char *flag_xyz);
+
+/* Launch-shape knobs of one context, for A/B measurements; they change no result beyond round-off.  Keys:
+ * "x_sweep" (0 automatic, 1 tile kernel, 2 marching kernel), "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a
+ * CTA of the viscous passes / the sensor marches; 0 automatic, else >= 8).  Unknown key or negative value: OCFD_EINVAL. */
+ocfd_status ocfd_set_tuning(ocfd_ctx *ctx, const char *key, int value);
 
 /* sizeof(ocfd_params) as compiled, so that a foreign-language mirror of the struct can check itself. */
 size_t ocfd_sizeof_params(void);

@@ -716,14 +716,9 @@ void ora_rhs(const ora_params *P, const double *U, double *dU) {
 
 /* Same L(U) at ONE interior point, computed from U alone with no stored intermediates, for sampled
  * parity on grids too large for ora_rhs.  tests/ check that it equals ora_rhs bit for bit. */
-static double theta_for(const ora_params *P, const double *U, int d, int i, int j, int k) {
-    return theta_ext(P, U, d, i, j, k);
-}
 static void fv_dir_at(const ora_params *P, const double *U, int d, int i, int j, int k, double out4[4]) {
     /* viscous flux of direction d at interior point (i,j,k), derivatives straight from U */
     double g[4][3], m[9];
-    long np = NP(P);
-    (void)np;
     for (int e = 0; e < 3; ++e) {
         long st = dim_stride(P, e);
         int s = e == 0 ? i : e == 1 ? j : k, n = dim_n(P, e);
@@ -762,7 +757,7 @@ void ora_rhs_point(const ora_params *P, const double *U, int i, int j, int k, do
             if (P->scheme == ORA_HYBRID) {
                 int a[3] = { i, j, k }, b[3] = { i, j, k };
                 a[d] = s0 - 1 + e; b[d] = s0 + e;
-                sch = iface_scheme(P, theta_for(P, U, d, a[0], a[1], a[2]), theta_for(P, U, d, b[0], b[1], b[2]));
+                sch = iface_scheme(P, theta_ext(P, U, d, a[0], a[1], a[2]), theta_ext(P, U, d, b[0], b[1], b[2]));
             }
             if (P->char_recon) {
                 double S[5][5], Si[5][5];
@@ -779,9 +774,6 @@ void ora_rhs_point(const ora_params *P, const double *U, int i, int j, int k, do
     }
     if (P->inviscid) return;
     double acc[4] = { 0, 0, 0, 0 };
-    for (int r = 0; r < 4; ++r) {
-        (void)r;
-    }
     double dsum[3][4];
     for (int d = 0; d < 3; ++d) {
         int c[3] = { i, j, k };

@@ -18,7 +18,7 @@ OCFD_OK = 0
 
 EXPORTS = ["ocfd_workspace_bytes", "ocfd_init", "ocfd_destroy", "ocfd_fill_ghosts", "ocfd_rhs", "ocfd_rk3_step",
            "ocfd_rk3_steps_host", "ocfd_max_wavespeed", "ocfd_debug_sensor", "ocfd_timing", "ocfd_timing_read",
-           "ocfd_kernel_name", "ocfd_sizeof_params", "ocfd_launch_count", "ocfd_strerror"]
+           "ocfd_kernel_name", "ocfd_sizeof_params", "ocfd_launch_count", "ocfd_strerror", "ocfd_set_tuning"]
 NKERNELS = 10
 
 
@@ -90,6 +90,8 @@ def load():
     L.ocfd_timing_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.ocfd_kernel_name.restype = C.c_char_p
     L.ocfd_kernel_name.argtypes = [C.c_int]
+    L.ocfd_set_tuning.restype = C.c_int
+    L.ocfd_set_tuning.argtypes = [vp, C.c_char_p, C.c_int]
     L.ocfd_sizeof_params.restype = C.c_size_t
     L.ocfd_sizeof_params.argtypes = []
     if L.ocfd_sizeof_params() != C.sizeof(OcfdParams):
@@ -242,6 +244,9 @@ class Solver:
         n = (C.c_longlong * NKERNELS)()
         _check(self.L.ocfd_timing_read(self.ctx, ms, n))
         return {self.L.ocfd_kernel_name(k).decode(): (ms[k], n[k]) for k in range(NKERNELS)}
+
+    def set_tuning(self, key, value):
+        _check(self.L.ocfd_set_tuning(self.ctx, key.encode(), int(value)))
 
     def launch_count(self):
         return int(self.L.ocfd_launch_count(self.ctx))

@@ -1,7 +1,6 @@
 // C ABI of libocfd_b200 (include/ocfd.h): argument validation, workspace carve-up, step orchestration.
 #include <math.h>
 #include <new>
-#include <stdlib.h>
 #include <string.h>
 
 #include "ocfd_internal.cuh"
@@ -16,6 +15,7 @@ bool valid_params(const ocfd_params *p) {
     if (!p) return false;
     if (p->ng != OCFD_NG) return false;
     if (p->nx < 8 || p->ny < 8 || p->nz < 8) return false;
+    if (p->nx > OCFD_MAX_EXTENT || p->ny > OCFD_MAX_EXTENT || p->nz > OCFD_MAX_EXTENT) return false;  // grid dimensions of the launches
     if (p->nx % 2) return false;  // TMA: row pitch (nx+8)*8 bytes must be a multiple of 16
     if ((long long)(p->nx + 8) * (p->ny + 8) * (p->nz + 8) > (1ll << 40)) return false;
     if (!(p->gamma > 1.0) || !(p->Ma > 0.0) || !(p->weno_eps > 0.0) || !(p->sw_eps >= 0.0)) return false;
@@ -24,7 +24,7 @@ bool valid_params(const ocfd_params *p) {
     if (p->visc_order != 0 && p->visc_order != 6 && p->visc_order != 8) return false;
     if (p->bc_closure != 0 && p->bc_closure != 1) return false;
     if (p->char_recon != 0 && p->char_recon != 1) return false;
-    if (p->scheme == OCFD_HYBRID && (isnan(p->theta1) || isnan(p->theta2))) return false;
+    if (p->scheme == OCFD_HYBRID && (isnan(p->theta1) || isnan(p->theta2) || p->theta1 > p->theta2)) return false;
     switch (p->grid_kind) {
         case OCFD_GRID_UNIFORM:
             if (!(p->dx > 0.0) || !(p->dy > 0.0) || !(p->dz > 0.0)) return false;
@@ -75,6 +75,17 @@ Carve carve(const ocfd_params *p) {
 
 bool live(const ocfd_ctx *c) { return c && c->magic == kMagic; }
 
+// x sweep: the marching kernel for the linear and hybrid schemes (4.4 against 4.75 ms on config 5), the tile kernel for
+// WENO everywhere (ALU-bound; the march has too few CTAs on grids with a short y axis) and for grids whose y-z
+// cross-section gives the march fewer than two waves of CTAs (32 y-lines each).  ocfd_set_tuning("x_sweep") overrides.
+void pick_x_sweep(ocfd_ctx *c) {
+    const ocfd_params &p = c->p;
+    c->x_tile = p.scheme == OCFD_WENO7 || p.scheme == OCFD_WENO5 ||
+                (long long)((p.ny + 31) / 32) * p.nz < 2ll * 3 * c->nsm;
+    if (c->tune.x_sweep == 1) c->x_tile = 1;
+    if (c->tune.x_sweep == 2) c->x_tile = 0;
+}
+
 }  // namespace
 
 extern "C" {
@@ -102,17 +113,8 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->p = *p;
     c->stream = (cudaStream_t)p->stream;
     c->nsm = nsm;
-    {
-        // x sweep: the marching kernel for the linear and hybrid schemes (4.4 against 4.75 ms on config 5), the tile kernel
-        // for WENO everywhere (ALU-bound; the march has too few CTAs on grids with a short y axis).  OCFD_X_SWEEP = tile
-        // or march overrides (A/B runs, profiles/r01_c_x_sweep_ab.md).
-        const char *e = getenv("OCFD_X_SWEEP");
-        // ... and for grids whose y-z cross-section gives the march fewer than two waves of CTAs (32 y-lines each)
-        c->x_tile = p->scheme == OCFD_WENO7 || p->scheme == OCFD_WENO5 ||
-                    (long long)((p->ny + 31) / 32) * p->nz < 2ll * 3 * nsm;
-        if (e && !strcmp(e, "tile")) c->x_tile = 1;
-        if (e && !strcmp(e, "march")) c->x_tile = 0;
-    }
+    c->tune = Tuning();
+    pick_x_sweep(c);
     c->visc_order = p->visc_order == 8 ? 8 : 6;
     GridDesc &g = c->g;
     g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
@@ -238,6 +240,9 @@ ocfd_status ocfd_debug_sensor(ocfd_ctx *c, const double *U, double *theta, unsig
     if (!live(c)) return OCFD_ESTATE;
     if (!U) return OCFD_EINVAL;
     ocfd_status st;
+    // all-ones bytes are a NaN: what the sensor does not write (everything but the interior and the first ghost layer
+    // of each face) comes back as NaN
+    if (cudaMemsetAsync(c->theta, 0xff, c->g.np * sizeof(double), c->stream) != cudaSuccess) return OCFD_ECUDA;
     if ((st = launch_prim(c, U)) != OCFD_OK) return st;
     if ((st = launch_sensor(c, U)) != OCFD_OK) return st;
     if (theta && cudaMemcpyAsync(theta, c->theta, c->g.np * sizeof(double), cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
@@ -276,6 +281,17 @@ const char *ocfd_kernel_name(int id) {
 }
 
 size_t ocfd_sizeof_params(void) { return sizeof(ocfd_params); }
+
+ocfd_status ocfd_set_tuning(ocfd_ctx *c, const char *key, int value) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!key || value < 0) return OCFD_EINVAL;
+    if (!strcmp(key, "x_sweep")) { if (value > 2) return OCFD_EINVAL; c->tune.x_sweep = value; pick_x_sweep(c); }
+    else if (!strcmp(key, "zchunk_flux")) c->tune.zchunk_f = value;
+    else if (!strcmp(key, "zchunk_div")) c->tune.zchunk_d = value;
+    else if (!strcmp(key, "zchunk_sensor")) c->tune.zchunk_s = value;
+    else return OCFD_EINVAL;
+    return OCFD_OK;
+}
 
 long long ocfd_launch_count(const ocfd_ctx *c) { return live(c) ? c->launches : -1; }
 

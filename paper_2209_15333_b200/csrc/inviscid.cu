@@ -220,8 +220,13 @@ __global__ void __launch_bounds__(INV_NT, CHAR ? 2 : 3)
                     wm[6] = fm[(q - q0 + 6) * ACP];
                     const int flag = SCHEME == OCFD_HYBRID ? (int)((mask >> (2 * (q - q0))) & 3u) : 0;
                     double h = 0.0;
-                    if (q < qlive && !CHAR)
-                        h = recon_pair_closure<SCHEME>(flag, o0 - 1 + q, nd, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6],
+                    // in characteristic variables phase B' redoes the interfaces inside the boundary band and the
+                    // non-linear ones; the linear interfaces of this segment outside the band stay with the walker
+                    const int s = o0 - 1 + q;
+                    const bool mine = !CHAR || ((SCHEME == OCFD_UD7 || (SCHEME == OCFD_HYBRID && flag == 0)) &&
+                                                !(s <= 2 || s >= nd - 4));
+                    if (q < qlive && mine)
+                        h = recon_pair_closure<SCHEME>(flag, s, nd, wp[0], wp[1], wp[2], wp[3], wp[4], wp[5], wp[6],
                                                        wm[6], wm[5], wm[4], wm[3], wm[2], wm[1], wm[0], gs.weno_eps);
                     sH[(m * NIF + q) * ACP + a] = h;
                 }
@@ -327,12 +332,7 @@ template <int KIND, int SCHEME, int DIR, bool CHAR>
 ocfd_status launch_dir(ocfd_ctx *c, const double *U) {
     const GridDesc &g = c->g;
     const size_t shm = TileGeom<DIR>::smem_bytes;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_inviscid<KIND, SCHEME, DIR, CHAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess)
-            return OCFD_ECUDA;
-        attr_set = true;
-    }
+    if (!ocfd_smem_optin(c, (const void *)k_inviscid<KIND, SCHEME, DIR, CHAR>, shm)) return OCFD_ECUDA;
     const int nd = DIR == 0 ? g.nx : DIR == 1 ? g.ny : g.nz;
     const int na = DIR == 0 ? g.ny : g.nx;
     const int ncross = DIR == 2 ? g.ny : g.nz;

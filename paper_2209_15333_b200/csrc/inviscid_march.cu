@@ -310,13 +310,7 @@ __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
 template <int KIND, int SCHEME, int DIR>
 ocfd_status launch_march(ocfd_ctx *c) {
     const GridDesc &g = c->g;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_inviscid_march<KIND, SCHEME, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)M_SMEM) != cudaSuccess)
-            return OCFD_ECUDA;
-        attr_set = true;
-    }
+    if (!ocfd_smem_optin(c, (const void *)k_inviscid_march<KIND, SCHEME, DIR>, M_SMEM)) return OCFD_ECUDA;
     const int ncross = DIR == 2 ? g.ny : g.nz;
     if (ncross > 65535) return OCFD_EINVAL;
     dim3 grd(((DIR == 0 ? g.ny : g.nx) + MAC - 1) / MAC, ncross, 1);

@@ -35,7 +35,7 @@ ocfd_status launch_metric_tables(ocfd_ctx *c) {
     if (g.kind == OCFD_GRID_CURVILINEAR) {
         const long long npts = g.atab_fs;
         int blocks = (int)((npts + 255) / 256);
-        if (blocks > 148 * 16) blocks = 148 * 16;
+        if (blocks > c->nsm * 16) blocks = c->nsm * 16;
         k_alpha_tables<<<blocks, 256, 0, c->stream>>>(g, c->mtab, npts);
         if (cudaGetLastError() != cudaSuccess) return OCFD_ECUDA;
     } else if (g.kind == OCFD_GRID_STRETCHED) {

@@ -72,6 +72,14 @@ struct ViscMaps {
     CUtensorMap prim, F, G, H, dU, U, Un;
 };
 
+// Tuning knobs of one context (ocfd_set_tuning): launch-shape choices that change no result beyond round-off.
+struct Tuning {
+    int x_sweep;     // 0 automatic, 1 tile kernel, 2 marching kernel
+    int zchunk_f;    // planes per CTA of viscous pass 1 (0 automatic)
+    int zchunk_d;    // ... of viscous pass 2
+    int zchunk_s;    // ... of the shock sensor
+};
+
 struct ocfd_ctx {
     uint64_t magic;
     ocfd_params p;
@@ -81,6 +89,8 @@ struct ocfd_ctx {
     int visc_order;  // 6 or 8 (ocfd_params.visc_order, 0 -> 6)
     int x_tile;      // x sweep by the tile kernel of inviscid.cu (1: default for WENO7 / WENO5) or the marching kernel (0: UD7, hybrid)
     int nsm;         // SM count of the device (persistent kernels launch a multiple of it)
+    Tuning tune;
+    std::vector<const void *> smem_optin;   // kernels whose dynamic shared-memory limit has been raised in this context
     // workspace carve-up (device pointers)
     double *prim;    // [6][np]: T u v w c p
     double *theta;   // [np]
@@ -201,6 +211,16 @@ ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int 
 ocfd_status launch_viscous(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage);
 ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage);
 ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
+
+// Raise the dynamic shared-memory limit of `kernel` to `bytes` once per context (the attribute lives in the device
+// context of the function, so a process-wide flag would leave a second device without it).
+inline bool ocfd_smem_optin(ocfd_ctx *c, const void *kernel, size_t bytes) {
+    for (const void *k : c->smem_optin)
+        if (k == kernel) return true;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) return false;
+    c->smem_optin.push_back(kernel);
+    return true;
+}
 
 // a failed launch is reported on stderr with the CUDA error text (the C ABI only carries OCFD_ECUDA)
 inline bool ocfd_launch_failed(const char *file, int line) {

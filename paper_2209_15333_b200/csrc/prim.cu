@@ -3,7 +3,6 @@
 #include "schemes.cuh"
 #include "tma.cuh"
 
-#include <stdlib.h>
 
 namespace {
 
@@ -153,6 +152,7 @@ __global__ void __launch_bounds__(256) k_wavespeed(GridDesc g, GasDesc gs, const
     long long n = (long long)g.nx * g.ny * g.nz;
     long long stride = (long long)gridDim.x * blockDim.x;
     double best = 0.0;
+    bool bad = false;
     for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) {
         int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long long)g.nx * g.ny));
         int ip = i + OCFD_NG, jp = j + OCFD_NG, kp = k + OCFD_NG;
@@ -168,11 +168,16 @@ __global__ void __launch_bounds__(256) k_wavespeed(GridDesc g, GasDesc gs, const
             Met<KIND>::row(g, d, ip, jp, kp, a1, a2, a3);
             s += fabs(a1 * u + a2 * v + a3 * w) + c * sqrt(a1 * a1 + a2 * a2 + a3 * a3);
         }
+        // fmax drops a NaN operand: a blown-up state (NaN rho or p) must not come back as a finite Lambda
+        bad |= !(s == s);
         best = fmax(best, s);
     }
-    // warp-shuffle max, then one atomic per warp on the ordered bit pattern (all values are >= 0)
+    // warp-shuffle max, then one atomic per warp on the ordered bit pattern (all values are >= 0; the quiet-NaN
+    // pattern orders above +inf, so one bad point makes the result NaN)
     for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
-    if ((threadIdx.x & 31) == 0) atomicMax(out, (unsigned long long)__double_as_longlong(best));
+    bad = __any_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0)
+        atomicMax(out, bad ? 0x7ff8000000000000ull : (unsigned long long)__double_as_longlong(best));
 }
 
 }  // namespace
@@ -202,9 +207,9 @@ ocfd_status launch_sensor(ocfd_ctx *c, const double *U) {
     // enough blocks to fill the SMs a few times over, chunks long enough that the two prologue planes stay cheap
     const long long tiles = (long long)((g.nx + ST - 1) / ST) * ((g.ny + SY - 1) / SY);
     int zc = g.nz;
-    while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < 148 * 16) zc = (zc + 1) / 2;
+    while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < c->nsm * 16) zc = (zc + 1) / 2;
     if (zc > 64) zc = 64;   // short marches keep halo-sharing tiles close in z (as in the viscous kernels; 0.64 -> 0.59 ms)
-    if (const char *e = getenv("OCFD_ZCHUNK_S")) { const int v = atoi(e); if (v >= 8) zc = v < g.nz ? v : g.nz; }
+    if (c->tune.zchunk_s >= 8) zc = c->tune.zchunk_s < g.nz ? c->tune.zchunk_s : g.nz;
     dim3 blk(ST, SY, 1), grd((g.nx + ST - 1) / ST, (g.ny + SY - 1) / SY, (g.nz + zc - 1) / zc);
     OCFD_T0(c, K_SENSOR);
     k_sensor<<<grd, blk, S_SMEM, c->stream>>>(g, c->sens_map, c->theta, zc);
@@ -227,7 +232,7 @@ ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out) {
     if (cudaMemsetAsync(out, 0, sizeof(unsigned long long), c->stream) != cudaSuccess) return OCFD_ECUDA;
     long long n = (long long)g.nx * g.ny * g.nz;
     int blocks = (int)((n + 255) / 256);
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > c->nsm * 16) blocks = c->nsm * 16;
     OCFD_T0(c, K_WAVE);
     switch (g.kind) {
         case OCFD_GRID_UNIFORM: k_wavespeed<OCFD_GRID_UNIFORM><<<blocks, 256, 0, c->stream>>>(g, c->gas, U, out); break;

@@ -13,7 +13,6 @@
 #include "schemes.cuh"
 #include "tma.cuh"
 
-#include <stdlib.h>
 
 namespace {
 
@@ -310,20 +309,19 @@ __global__ void __launch_bounds__(VNT, 1)
     }
 }
 
-int pick_zchunk(const GridDesc &g, int pass) {
-    // enough blocks to fill 148 SMs a few times over ...
+int pick_zchunk(const ocfd_ctx *c, int pass) {
+    const GridDesc &g = c->g;
+    // enough blocks to fill the SMs a few times over ...
     const long long tiles = (long long)((g.nx + TX - 1) / TX) * ((g.ny + TY - 1) / TY);
     int zc = g.nz;
-    while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < 148 * 8) zc = (zc + 1) / 2;
+    while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < c->nsm * 8) zc = (zc + 1) / 2;
     // ... and short enough that tiles which share a halo stay close in z: CTAs drift apart while they march, and a
     // halo plane the neighbour read long ago has left the L2.  Measured on config 5 (profiles/r01_c): chunks of 64
     // planes for pass 1 (4.94 -> 4.73 ms) and 32 for pass 2 (7.99 -> 7.02 ms); the prologue planes of a chunk come from L2.
     const int cap = pass == 1 ? 64 : 32;
     if (zc > cap) zc = cap;
-    if (const char *e = getenv(pass == 1 ? "OCFD_ZCHUNK_F" : "OCFD_ZCHUNK_D")) {   // tuning knob for A/B runs
-        const int v = atoi(e);
-        if (v >= 8) zc = v < g.nz ? v : g.nz;
-    }
+    const int v = pass == 1 ? c->tune.zchunk_f : c->tune.zchunk_d;   // ocfd_set_tuning (A/B runs)
+    if (v >= 8) zc = v < g.nz ? v : g.nz;
     return zc;
 }
 
@@ -355,13 +353,7 @@ bool encode_maps(ocfd_ctx *c, const double *dU, const double *U) {
 
 template <int KIND, int RK, int ORDER>
 ocfd_status launch_div(ocfd_ctx *c, dim3 grd, dim3 blk, double *dU, double *U, double dt, int zc) {
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_viscous_div<KIND, RK, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)VD<ORDER>::SMEM) != cudaSuccess)
-            return OCFD_ECUDA;
-        attr_set = true;
-    }
+    if (!ocfd_smem_optin(c, (const void *)k_viscous_div<KIND, RK, ORDER>, VD<ORDER>::SMEM)) return OCFD_ECUDA;
     const ViscMaps &M = c->visc;
     k_viscous_div<KIND, RK, ORDER><<<grd, blk, VD<ORDER>::SMEM, c->stream>>>(c->g, M.F, M.G, M.H, M.dU, RK ? M.U : M.dU, M.Un, c->Fv, dU, U,
                                                              c->Un, dt, zc);
@@ -372,14 +364,8 @@ template <int KIND, int ORDER>
 ocfd_status launch_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
     const GridDesc &g = c->g;
     if (!encode_maps(c, dU, rk_stage >= 0 ? U : nullptr)) return OCFD_ECUDA;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(k_viscous_flux<KIND, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)VF<ORDER>::SMEM) != cudaSuccess)
-            return OCFD_ECUDA;
-        attr_set = true;
-    }
-    const int zc = pick_zchunk(g, 1), zcd = pick_zchunk(g, 2);
+    if (!ocfd_smem_optin(c, (const void *)k_viscous_flux<KIND, ORDER>, VF<ORDER>::SMEM)) return OCFD_ECUDA;
+    const int zc = pick_zchunk(c, 1), zcd = pick_zchunk(c, 2);
     dim3 blk(TX, TY, 1), grd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zc - 1) / zc);
     dim3 grdd(grd.x, grd.y, (g.nz + zcd - 1) / zcd);
     OCFD_T0(c, K_VISC_FLUX);

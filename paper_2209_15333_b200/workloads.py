@@ -283,11 +283,16 @@ def flat_plate(nx=1024, ny=128, nz=128, seed=20224, scheme="weno7", nsteps=50, L
 
 # --------------------------------------------------------------------------- config 5: ramp
 def ramp(nx=2048, ny=300, nz=256, seed=20225, scheme="hybrid", theta2=np.inf, nsteps=20, dz=0.1,
-         x0=-120.0, x1=84.8, H=60.0, dy1=0.004, nmodes=64, rms=0.05):
+         x0=-120.0, x1=84.8, H=60.0, dy1=0.004, nmodes=64, rms=0.05, nshocks=1):
     """Mach 2.9, 24-degree compression-ramp-shaped curvilinear grid, z-extruded 2-D map (config 5).
 
     Wall y_w(x) = tan24 (x + sqrt(x^2 + d^2))/2 - tan24 d/2 (smoothed corner, d = 2), x uniform,
-    y = y_w + (H - y_w) g(eta), tanh clustering g as config 4; metrics analytic via eq. 3-4."""
+    y = y_w + (H - y_w) g(eta), tanh clustering g as config 4; metrics analytic via eq. 3-4.
+
+    nshocks > 1 adds a train of nshocks - 1 weak oblique fronts upstream of the ramp shock (normal Mach numbers 1.05 to
+    1.35, Rankine-Hugoniot jumps, smeared like the main shock): a stand-in for the shocklets / shock systems that make
+    "up to 10 %" of the interfaces leave the linear scheme, used by the bench workloads that measure the
+    hybrid kernels at that flagged fraction.  nshocks = 1 is BASELINE.json's config 5."""
     gamma, Ma, Re, Pr, T_ref = 1.4, 2.9, 5600.0, 0.72, 108.1
     Tw = 1.0 + np.sqrt(Pr) * 0.5 * (gamma - 1.0) * Ma * Ma
     dxx = (x1 - x0) / nx
@@ -358,6 +363,18 @@ def ramp(nx=2048, ny=300, nz=256, seed=20225, scheme="hybrid", theta2=np.inf, ns
     dsh = (np.tan(beta) * xs[None, :] - Y) * np.cos(beta)              # > 0 behind the shock
     sh = 0.5 * (1.0 + np.tanh(dsh / (1.5 * dxx)))
     fp_, ft_, fv_ = 1.0 + (p_ratio - 1.0) * sh, 1.0 + (p_ratio / r_ratio - 1.0) * sh, 1.0 + (v_ratio - 1.0) * sh
+    for q in range(1, nshocks):
+        m1n = 1.05 + 0.1 * (q % 4)                                      # normal Mach number of front q
+        bq = np.arcsin(m1n / Ma)
+        pq = 1.0 + 2.0 * gamma / (gamma + 1.0) * (m1n ** 2 - 1.0)
+        rq = (gamma + 1.0) * m1n ** 2 / ((gamma - 1.0) * m1n ** 2 + 2.0)
+        vq = np.sqrt(np.cos(bq) ** 2 + (np.sin(bq) / rq) ** 2)
+        xq = -q * 110.0 / nshocks                                       # foot of the front on the plate, upstream
+        dq = (np.tan(bq) * (xs[None, :] - xq) - Y) * np.cos(bq)
+        sq = 0.5 * (1.0 + np.tanh(dq / (1.5 * dxx)))
+        fp_ = fp_ * (1.0 + (pq - 1.0) * sq)
+        ft_ = ft_ * (1.0 + (pq / rq - 1.0) * sq)
+        fv_ = fv_ * (1.0 + (vq - 1.0) * sq)
     u *= fv_[None]
     v *= fv_[None]
     w *= fv_[None]
@@ -496,13 +513,14 @@ def sod(n=200, scheme="weno7", ny=4, nz=4):
                 U0=np.ascontiguousarray(U), coords=(x, None, None))
 
 
-def shocked_periodic(n=24, seed=11, scheme="hybrid", theta1=0.02, theta2=0.1):
+def shocked_periodic(n=24, seed=11, scheme="hybrid", theta1=0.02, theta2=0.1, steep=6.0):
     """Periodic box with a smooth background plus steep pressure/density fronts, so that all three
-    levels of the hybrid scheme are exercised."""
+    levels of the hybrid scheme are exercised.  `steep` sets the front thickness (in units of the box,
+    so a bench-sized box passes steep ~ n/7 to keep the fronts a few cells thick)."""
     c = smooth_periodic(n, n, n, seed=seed, scheme=scheme, Ma=1.2, amp=0.15, inviscid=False)
     KK, JJ, II = np.meshgrid(_idx(n), _idx(n), _idx(n), indexing="ij")
     s = 2 * np.pi / n
-    front = 0.5 * (1.0 + np.tanh(6.0 * np.sin(s * II + 0.7 * np.sin(s * JJ)) * np.cos(s * KK * 1.0 + 0.3)))
+    front = 0.5 * (1.0 + np.tanh(steep * np.sin(s * II + 0.7 * np.sin(s * JJ)) * np.cos(s * KK * 1.0 + 0.3)))
     U = c.U0.copy()
     fac = 1.0 + 1.5 * front
     U[0] *= fac

@@ -1,0 +1,73 @@
+"""Multi-step parity of the five BASELINE.json configs at the sizes SURVEY 8(d) names for the oracle: config 1 and 2 in
+full (32^3 x 10 steps is in test_gpu_parity.py; 128^3 x 100 steps here), config 3 on its 128^3 twin x 50 steps, config 4
+on 256 x 64 x 32 x 50 steps, config 5 on 512 x 76 x 32 x 20 steps, all through ocfd_rk3_step (the fused path bench.py
+times) against the oracle stepped on the host cores.
+
+Bar (north_star): <= 1e-9 relative L-inf of U after the steps on smooth cases.  Hybrid cases: the sensor decisions of
+the two sides are compared at every step (mismatches outside the 1e-12 band must be 0, those inside are counted), and
+every interface whose Theta comes within 1e-9 of a threshold at ANY stage on the oracle side is recorded; the 1e-9 bar
+is then asserted on all points outside the domain of influence of those interfaces, and the counts are printed (no
+loosened tolerance: tests/parity_utils.py:step_both_hybrid).
+"""
+import numpy as np
+import pytest
+
+from paper_2209_15333_b200 import workloads as W
+from tests.parity_utils import step_both_hybrid
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEPS = 1e-9
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_2209_15333_b200 import binding
+    binding.load()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def Oracle():
+    from oracle.oracle import Oracle
+    return Oracle
+
+
+def check(res, smooth):
+    assert res["finite"]
+    assert res["flag_mismatches"] == 0
+    if smooth or res["near"] == 0:
+        assert res["err_all"] <= TOL_STEPS, res
+    else:
+        assert res["excluded_fraction"] < 1.0, "every point lies in the domain of influence of a near-threshold interface"
+        assert res["err_outside"] <= TOL_STEPS, res
+
+
+def test_config2_hit128_weno7_hundred_steps(B, Oracle):
+    case = W.hit(128)                                   # WENO7, Mt 0.5, 100 steps (BASELINE.json configs[1])
+    assert (case.nx, case.scheme, case.nsteps) == (128, "weno7", 100)
+    check(step_both_hybrid(B, Oracle, case, 100), smooth=True)
+
+
+@pytest.mark.parametrize("theta2", [np.inf, 0.1])
+def test_config3_shocklet_hit_twin128_hybrid_fifty_steps(B, Oracle, theta2):
+    case = W.hit(128, Mt=1.0, seed=20223, scheme="hybrid", nsteps=50, theta2=theta2)
+    res = step_both_hybrid(B, Oracle, case, 50, check_flags_every=10)
+    check(res, smooth=False)
+    assert res["hist0"][0] > 0                          # the linear scheme is what most interfaces take
+
+
+def test_config4_flat_plate_twin_weno7_fifty_steps(B, Oracle):
+    case = W.flat_plate(nx=256, ny=64, nz=32)           # 256 x 64 x 32 twin, 50 steps
+    check(step_both_hybrid(B, Oracle, case, 50), smooth=True)
+
+
+@pytest.mark.parametrize("theta2", [np.inf, 0.1])
+def test_config5_ramp_twin_hybrid_twenty_steps(B, Oracle, theta2):
+    case = W.ramp(nx=512, ny=76, nz=32, theta2=theta2)  # 512 x 76 x 32 twin, 20 steps
+    res = step_both_hybrid(B, Oracle, case, 20, check_flags_every=5)
+    check(res, smooth=False)
+    assert res["hist0"][1] > 0                          # the oblique shock of the generator is flagged

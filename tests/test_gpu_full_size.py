@@ -93,6 +93,45 @@ def test_config3_shocklet_hit256_full_size_sampled(B, Oracle):
     assert err.max() <= TOL_RHS
 
 
+def full_size_flag_report(B, Oracle, case):
+    """ocfd_debug_sensor against ora_sensor / ora_flags on the whole grid (north_star: decisions must match at every
+    point except those within 1e-12 of a threshold, which are counted and reported; eq. 42)."""
+    import torch
+    from tests.parity_utils import compare_flags
+    o = Oracle(case)
+    U = o.fill_ghosts(case.U0.copy())
+    th_ref = o.sensor(U)
+    fl_ref = [o.flags(th_ref, d) for d in range(3)]
+    s = B.Solver(case)
+    Ud = s.to_device(U)
+    del U
+    th_gpu, fl_gpu = s.debug_sensor(Ud)
+    torch.cuda.synchronize()
+    I = slice(NG, -NG)
+    dth = float((th_gpu[I, I, I].cpu() - torch.from_numpy(th_ref[I, I, I])).abs().max())
+    fl_gpu = fl_gpu.cpu().numpy()
+    del th_gpu, Ud
+    s.close()
+    bad, near, total, hist = compare_flags(th_ref, fl_ref, fl_gpu, case.theta1, case.theta2)
+    print(f"{case.name}: {total} interfaces, max |theta_gpu - theta_ora| {dth:.2e}, {near} within 1e-12 of a threshold "
+          f"(excluded), {bad} mismatches outside the band; UD7/WENO7/WENO5 = {hist.tolist()} "
+          f"({100.0 * (hist[1] + hist[2]) / hist.sum():.2f} % flagged)")
+    assert dth <= 1e-13
+    assert bad == 0
+    return hist
+
+
+@pytest.mark.parametrize("theta2", [np.inf, 0.1])
+def test_config5_ramp_full_size_sensor_decisions(B, Oracle, theta2):
+    hist = full_size_flag_report(B, Oracle, W.ramp(theta2=theta2))
+    assert hist[1] > 0 and (np.isinf(theta2) or hist[2] > 0)
+
+
+@pytest.mark.parametrize("theta2", [np.inf, 0.1])
+def test_config3_shocklet_hit256_full_size_sensor_decisions(B, Oracle, theta2):
+    full_size_flag_report(B, Oracle, W.hit(256, Mt=1.0, seed=20223, scheme="hybrid", nsteps=50, theta2=theta2))
+
+
 def test_config2_hit128_whole_array_rhs_and_three_steps(B, Oracle):
     case = W.hit(128)                                              # WENO7
     o = Oracle(case)

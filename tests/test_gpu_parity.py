@@ -4,6 +4,9 @@ Tolerances (BASELINE.json north_star): relative L-inf <= 1e-11 per RHS, <= 1e-9 
 cases; hybrid-scheme flags exact except within 1e-12 of a threshold (counted and reported).
 Error metric (SURVEY 8(c)): per conserved component m, max_i |gpu - ora| / max_i |ora| over interior points;
 when max|ora_m| is (numerically) zero the error is taken relative to max|U_m|.
+DESIGN.md reading R-23 extends "numerically zero" to "zero by cancellation": a component whose max|ora_m| lies below
+1e-3 * Lambda * max|U| (0.1 % of the size of the terms that sum to it) is measured against that floor.  Every test that
+uses the floor prints the un-floored error of every component beside the floored one and says which were floored.
 """
 import numpy as np
 import pytest
@@ -51,6 +54,16 @@ def rel_linf(gpu, ora, U, floor=0.0):
 
 def term_floor(Oracle, case, U_full):
     return 1e-3 * Oracle(case).max_wavespeed(U_full) * np.abs(U_full[INT]).max()
+
+
+def report(tag, got, ref, U, floor):
+    """Print the un-floored error of every component beside the floored one (DESIGN R-23); returns the floored errors."""
+    raw = rel_linf(got, ref, U)
+    flo = rel_linf(got, ref, U, floor)
+    which = [m for m in range(5) if np.abs(ref[m]).max() < floor]
+    print(f"{tag}: rel Linf per component un-floored {raw}, floored {flo}; floor {floor:.3e}, max|ora| "
+          f"{np.abs(ref).reshape(5, -1).max(axis=1)}, components measured against the floor: {which}")
+    return flo
 
 
 def run_rhs_both(B, Oracle, case, fill=True):
@@ -172,8 +185,7 @@ def test_rhs_parity_with_walls(B, Oracle, which):
         case = W.ramp(nx=64, ny=44, nz=24, nmodes=12, theta2=np.inf if which == "ramp" else 0.1)
     got, ref, U = run_rhs_both(B, Oracle, case)
     floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
-    err = rel_linf(got, ref, U, floor)
-    print(which, "rel Linf per component", err, "floor", floor, "max|ref|", np.abs(ref).max(axis=(1, 2, 3)))
+    err = report(f"walls/{which}", got, ref, U, floor)
     assert err.max() <= TOL_RHS
 
 
@@ -189,7 +201,7 @@ def test_rhs_parity_eighth_order_viscous_scheme(B, Oracle, which):
     case.visc_order = 8
     got, ref, U = run_rhs_both(B, Oracle, case)
     floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
-    err = rel_linf(got, ref, U, floor)
+    err = report(f"visc8/{which}", got, ref, U, floor)
     assert err.max() <= TOL_RHS
     case.visc_order = 6          # and the two schemes really differ
     ref6 = Oracle(case).rhs(Oracle(case).fill_ghosts(case.U0.copy()))[INT]
@@ -210,8 +222,7 @@ def test_rhs_parity_paper_boundary_scheme(B, Oracle, which):
     case.bc_closure = 1
     got, ref, U = run_rhs_both(B, Oracle, case)
     floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
-    err = rel_linf(got, ref, U, floor)
-    print(which, "rel Linf per component", err)
+    err = report(f"closure/{which}", got, ref, U, floor)
     assert err.max() <= TOL_RHS
     case.bc_closure = 0                # and the closure really changes the result
     o = Oracle(case)
@@ -229,7 +240,8 @@ def test_twenty_steps_paper_boundary_scheme(B, Oracle):
 
 
 @pytest.mark.parametrize("which", ["wavy-ud7", "wavy-weno7", "wavy-weno5", "stretched-hybrid", "uniform-weno7",
-                                   "shocked", "plate", "ramp3level", "box-closure"])
+                                   "shocked", "plate", "ramp3level", "box-closure", "box-closure-ud7",
+                                   "box-closure-hybrid", "plate-closure-ud7", "ramp-closure-hybrid"])
 def test_rhs_parity_characteristic_reconstruction(B, Oracle, which):
     """char_recon = 1 (PAPER.md:L212-263, SURVEY 8(f) NEXT #2): all three sweeps in characteristic variables."""
     if which == "plate":
@@ -238,9 +250,18 @@ def test_rhs_parity_characteristic_reconstruction(B, Oracle, which):
         case = W.ramp(nx=64, ny=44, nz=24, nmodes=12, theta2=0.1)
     elif which == "shocked":
         case = W.shocked_periodic(44, theta1=0.02, theta2=0.1)
-    elif which == "box-closure":
-        case = W.smooth_periodic(70, 45, 23, grid="wavy", scheme="weno7", Re=150.0, seed=6)
+    elif which.startswith("box-closure"):
+        # the paper's boundary scheme together with characteristic variables, for the linear and hybrid schemes too:
+        # the linear interfaces of a boundary segment that lie outside the boundary band stay with the walkers
+        scheme = which.split("-")[2] if which.count("-") == 2 else "weno7"
+        case = W.smooth_periodic(70, 45, 23, grid="wavy", scheme=scheme, Re=150.0, seed=6)
         case.bc = ["outflow"] * 6
+        case.bc_closure = 1
+    elif which == "plate-closure-ud7":
+        case = W.flat_plate(nx=72, ny=44, nz=24, scheme="ud7")
+        case.bc_closure = 1
+    elif which == "ramp-closure-hybrid":
+        case = W.ramp(nx=64, ny=44, nz=24, nmodes=12, theta2=0.1)
         case.bc_closure = 1
     else:
         grid, scheme = which.split("-")
@@ -248,8 +269,7 @@ def test_rhs_parity_characteristic_reconstruction(B, Oracle, which):
     case.char_recon = 1
     got, ref, U = run_rhs_both(B, Oracle, case)
     floor = term_floor(Oracle, case, Oracle(case).fill_ghosts(case.U0.copy()))
-    err = rel_linf(got, ref, U, floor)
-    print(which, "rel Linf per component", err)
+    err = report(f"char/{which}", got, ref, U, floor)
     assert err.max() <= TOL_RHS
 
 
@@ -296,6 +316,59 @@ def test_max_wavespeed_matches_the_oracle(B, Oracle, which):
     lam = s.max_wavespeed(s.to_device(U))
     s.close()
     assert lam == pytest.approx(o.max_wavespeed(U), rel=1e-13)
+
+
+def test_max_wavespeed_reports_a_blown_up_state_as_nan(B):
+    """A NaN anywhere in the interior must not come back as a finite Lambda (a caller would go on with a finite dt)."""
+    case = W.smooth_periodic(24, 16, 12, grid="wavy")
+    s = B.Solver(case)
+    U = case.U0.copy()
+    assert np.isfinite(s.max_wavespeed(s.to_device(U)))
+    U[4, NG + 5, NG + 7, NG + 11] = np.nan                 # E of one interior point
+    assert np.isnan(s.max_wavespeed(s.to_device(U)))
+    U = case.U0.copy()
+    U[0, NG + 1, NG + 2, NG + 3] = np.nan                  # rho
+    assert np.isnan(s.max_wavespeed(s.to_device(U)))
+    s.close()
+
+
+def test_two_contexts_in_one_process_do_not_share_state(B, Oracle):
+    """include/ocfd.h: "no global state; several contexts may coexist".  Two contexts with different grids, schemes and
+    kernel instantiations, created, used alternately and destroyed in one process (the shared-memory opt-in of the
+    kernels is kept per context)."""
+    a = W.ramp(nx=48, ny=30, nz=10, nmodes=8)
+    b = W.smooth_periodic(40, 24, 18, grid="stretched", scheme="weno7", Re=150.0, seed=4)
+    sa, sb = B.Solver(a), B.Solver(b)
+    refs, gots = [], []
+    for case, s in ((a, sa), (b, sb), (a, sa), (b, sb)):
+        o = Oracle(case)
+        U = o.fill_ghosts(case.U0.copy())
+        refs.append(o.rhs(U)[INT])
+        gots.append(s.rhs(s.to_device(U)).cpu().numpy()[INT])
+    sa.close()
+    sc = B.Solver(a)                                       # a new context after one was destroyed
+    U = Oracle(a).fill_ghosts(a.U0.copy())
+    gots.append(sc.rhs(sc.to_device(U)).cpu().numpy()[INT])
+    refs.append(refs[0])
+    sb.close()
+    sc.close()
+    for got, ref, case in zip(gots, refs, (a, b, a, b, a)):
+        U = Oracle(case).fill_ghosts(case.U0.copy())
+        floor = term_floor(Oracle, case, U)
+        assert rel_linf(got, ref, U[INT], floor).max() <= TOL_RHS
+    assert np.array_equal(gots[0], gots[2]) and np.array_equal(gots[1], gots[3]) and np.array_equal(gots[0], gots[4])
+
+
+def test_debug_sensor_leaves_nan_where_the_sensor_does_not_write(B):
+    case = W.shocked_periodic(20)
+    s = B.Solver(case)
+    th, fl = s.debug_sensor(s.fill_ghosts(s.to_device(case.U0.copy())))
+    th = th.cpu().numpy()
+    s.close()
+    I = slice(NG, -NG)
+    assert np.isfinite(th[I, I, I]).all()
+    assert np.isfinite(th[NG - 1, I, I]).all() and np.isfinite(th[I, -NG, I]).all() and np.isfinite(th[I, I, NG - 1]).all()
+    assert np.isnan(th[0]).all() and np.isnan(th[:, :, 0]).all() and np.isnan(th[NG - 1, NG - 1, :]).all()
 
 
 def test_results_are_bitwise_reproducible(B):
@@ -386,11 +459,19 @@ def test_hundred_steps_smooth(B, Oracle):
     assert err <= TOL_100
 
 
-@pytest.mark.parametrize("which", ["plate", "ramp"])
+@pytest.mark.parametrize("which", ["plate", "ramp", "ramp3level"])
 def test_twenty_steps_with_walls(B, Oracle, which):
-    case = W.flat_plate(nx=64, ny=40, nz=16) if which == "plate" else W.ramp(nx=64, ny=40, nz=16, nmodes=12)
-    err, got, ref = step_both(B, Oracle, case, 20)
-    print(which, "20 steps: rel Linf", err)
-    # hybrid decisions may legitimately flip where theta sits within round-off of a threshold; smooth twins stay tight
-    assert err <= (1e-9 if which == "plate" else 1e-7)
-    assert np.isfinite(got).all()
+    """20 steps with wall / inflow / outflow faces.  The hybrid cases carry no loosened bar: every interface whose Theta
+    comes within 1e-9 of a threshold at any stage is counted, and the 1e-9 bar holds outside its domain of influence
+    (everywhere when there is none); the sensor decisions of the two sides are compared at every step."""
+    from tests.parity_utils import step_both_hybrid
+    if which == "plate":
+        case = W.flat_plate(nx=64, ny=40, nz=16)
+    else:
+        case = W.ramp(nx=64, ny=40, nz=16, nmodes=12, theta2=np.inf if which == "ramp" else 0.1)
+    res = step_both_hybrid(B, Oracle, case, 20)
+    assert res["finite"] and res["flag_mismatches"] == 0
+    if res["near"] == 0:
+        assert res["err_all"] <= TOL_100, res
+    else:
+        assert res["excluded_fraction"] < 1.0 and res["err_outside"] <= TOL_100, res

@@ -103,12 +103,23 @@ def test_mirror_symmetry_pins_the_negative_flux_stencil(scheme):
     assert np.abs(dUr[INT] - ref[INT]).max() <= 1e-12 * np.abs(ref[INT]).max()
 
 
-def test_rhs_point_equals_rhs_everywhere_small():
-    for bc_case in ("periodic", "plate"):
+@pytest.mark.parametrize("option", ["default", "char_recon", "bc_closure", "visc_order8", "all"])
+def test_rhs_point_equals_rhs_everywhere_small(option):
+    """ora_rhs_point (the sampled-parity entry) is ora_rhs bit for bit, with every option the full-size GPU tests may
+    switch on: characteristic variables, the paper's boundary scheme, the 8th-order viscous scheme."""
+    for bc_case in ("periodic", "plate", "ramp"):
         if bc_case == "periodic":
             case = W.shocked_periodic(10)
-        else:
+        elif bc_case == "plate":
             case = W.flat_plate(nx=12, ny=10, nz=8, scheme="hybrid")
+        else:
+            case = W.ramp(nx=12, ny=10, nz=8, nmodes=4, theta2=0.1)
+        if option in ("char_recon", "all"):
+            case.char_recon = 1
+        if option in ("bc_closure", "all"):
+            case.bc_closure = 1
+        if option in ("visc_order8", "all"):
+            case.visc_order = 8
         o = Oracle(case)
         U = o.fill_ghosts(case.U0.copy())
         dU = o.rhs(U)
