@@ -3,8 +3,8 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl ours|reference]
 
-A "step" is one TVD-RK3 step (3 x [ghost fill, primitives, sensor, inviscid x/y/z, viscous flux/div, RK update] + a
-final ghost fill) of the whole hot path on one synthetic workload.  The default workload is
+A "step" is one TVD-RK3 step (3 x [ghost fill, viscous flux + sensor, inviscid x-y, inviscid z, viscous divergence +
+RK update] + a final ghost fill) of the whole hot path on one synthetic workload.  The default workload is
 BASELINE.json's configs[4], the >=100M-point Mach 2.9 ramp grid that north_star's target names; it fits one GPU.
 N > 1 runs N independent replicas (north_star: no domain decomposition), value = sum over replicas.
 Prints ONE JSON line on rank 0 (contract: see the task statement; extra keys: roofline, cpu_baseline, kernels).
@@ -119,19 +119,23 @@ def algorithmic(case, flag_hist=None):
         fl_rec = h[0] * rec["ud7"] + h[1] * rec["weno7"] + h[2] * rec["weno5"]
     else:
         fl_rec = rec[case.scheme]
-    inv_flops = 10 * fl_rec + 5 + 140 + 15
+    prim_flops = 30.0                   # row a2 inside a consumer: 1/rho, u, v, w, p, c (or T)
+    inv_flops = 10 * fl_rec + 5 + 140 + 15 + prim_flops
     th = 8 if hyb else 0
-    m_inv = 32 if met3d else 0
-    state = 8 + 32                      # rho from U, (u,v,w,c) from the primitive fields
+    m_inv = 40 if met3d else 0          # k1, k2, k3, sigma, J of one direction (z-extruded grids: L2-resident planes)
+    state = 40                          # the five conserved fields (no primitive field exists in HBM)
     out = {
         "ghost_fill": (0.0, 0.0),
-        "primitives": (88.0 * P, 25.0 * P),
-        "shock_sensor": (16.0, 25.0),
-        # x sweep writes dU; y / z sweeps add into it (TMA reduce at the L2: dU still crosses HBM in and out)
+        "shock_sensor": (40.0 + 8.0, 25.0 + prim_flops),      # stand-alone form (runs without viscous terms)
+        # x and y sweeps fused: the state is read once and dU written once for both directions
+        "inviscid_xy": (state + th + 2 * m_inv + 40, 2 * (10 * fl_rec + 5 + 140 + 15) + prim_flops),
+        # one launch per direction (characteristic variables, and the unfused reference): x writes dU, y / z add into it
+        # (TMA reduce at the L2: dU still crosses HBM in and out)
         "inviscid_x": (state + th + m_inv + 40, inv_flops),
         "inviscid_y": (state + th + m_inv + 80, inv_flops),
         "inviscid_z": (state + th + m_inv + 80, inv_flops),
-        "viscous_flux": (32 + 96 + (80 if met3d else 0), 240.0),
+        # a6 (+ a3 for the hybrid scheme: theta is written by this kernel, its inputs are already staged)
+        "viscous_flux": (40 + 96 + th + (80 if met3d else 0), 240.0 + prim_flops + (25.0 if hyb else 0.0)),
         # a7 + a8 fused (inside ocfd_rk3_step): R Fv 96 + dU 40 + U 40 + U^n 40 (W at stage 1), W U 40
         "viscous_div": (96 + 40 + 40 + 40 + 40 + (8 if met3d else 0), 125.0 + 20.0),
         "rk3_update": (160.0, 20.0),

@@ -141,8 +141,9 @@ ocfd_status ocfd_max_wavespeed(ocfd_ctx *ctx, const double *U, double *host_out)
 ocfd_status ocfd_debug_sensor(ocfd_ctx *ctx, const double *U, double *theta, unsigned char *flag_xyz);
 
 /* Launch-shape knobs of one context, for A/B measurements; they change no result beyond round-off.  Keys:
- * "x_sweep" (0 automatic, 1 tile kernel, 2 marching kernel), "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a
- * CTA of the viscous passes / the sensor marches; 0 automatic, else >= 8).  Unknown key or negative value: OCFD_EINVAL. */
+ * "xy_fused" (1, default: the x and y sweeps run as one kernel; 0: one marching launch per direction, the unfused
+ * reference), "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a CTA of the viscous passes / the stand-alone sensor
+ * marches; 0 automatic, else >= 8).  Unknown key or negative value: OCFD_EINVAL. */
 ocfd_status ocfd_set_tuning(ocfd_ctx *ctx, const char *key, int value);
 
 /* sizeof(ocfd_params) as compiled, so that a foreign-language mirror of the struct can check itself. */

@@ -49,14 +49,13 @@ bool valid_params(const ocfd_params *p) {
     return true;
 }
 
-struct Carve { size_t prim, theta, Fv, Un, dUw, scal, mtab, total; };
+struct Carve { size_t theta, Fv, Un, dUw, scal, mtab, total; };
 
 Carve carve(const ocfd_params *p) {
     const size_t np = (size_t)(p->nx + 8) * (p->ny + 8) * (p->nz + 8);
     const size_t fb = align_up(np * sizeof(double), 256);
     Carve c;
     size_t off = 0;
-    c.prim = off; off += align_up(P_NF * np * sizeof(double), 256);
     c.theta = off; off += fb;
     c.Fv = off; off += p->inviscid ? 0 : align_up(12 * np * sizeof(double), 256);
     c.Un = off; off += align_up(5 * np * sizeof(double), 256);
@@ -74,17 +73,6 @@ Carve carve(const ocfd_params *p) {
 }
 
 bool live(const ocfd_ctx *c) { return c && c->magic == kMagic; }
-
-// x sweep: the marching kernel for the linear and hybrid schemes (4.4 against 4.75 ms on config 5), the tile kernel for
-// WENO everywhere (ALU-bound; the march has too few CTAs on grids with a short y axis) and for grids whose y-z
-// cross-section gives the march fewer than two waves of CTAs (32 y-lines each).  ocfd_set_tuning("x_sweep") overrides.
-void pick_x_sweep(ocfd_ctx *c) {
-    const ocfd_params &p = c->p;
-    c->x_tile = p.scheme == OCFD_WENO7 || p.scheme == OCFD_WENO5 ||
-                (long long)((p.ny + 31) / 32) * p.nz < 2ll * 3 * c->nsm;
-    if (c->tune.x_sweep == 1) c->x_tile = 1;
-    if (c->tune.x_sweep == 2) c->x_tile = 0;
-}
 
 }  // namespace
 
@@ -114,7 +102,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->stream = (cudaStream_t)p->stream;
     c->nsm = nsm;
     c->tune = Tuning();
-    pick_x_sweep(c);
+    c->tune.xy_fused = 1;
     c->visc_order = p->visc_order == 8 ? 8 : 6;
     GridDesc &g = c->g;
     g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
@@ -141,7 +129,6 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     s.kfac = p->inviscid ? 0.0 : 1.0 / ((p->gamma - 1.0) * p->Ma * p->Ma * p->Pr * p->Re);
     s.weno_eps = p->weno_eps; s.sw_eps = p->sw_eps; s.theta1 = p->theta1; s.theta2 = p->theta2;
     char *w = (char *)p->workspace;
-    c->prim = (double *)(w + cv.prim);
     c->theta = (double *)(w + cv.theta);
     c->Fv = (double *)(w + cv.Fv);
     c->Un = (double *)(w + cv.Un);
@@ -161,12 +148,14 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->flags = nullptr;
     c->launches = 0;
     c->inv.ready = false;
-    c->inv.U = c->inv.dU = nullptr;
+    c->inv.Up = c->inv.dUp = nullptr;
     c->march.ready = false;
-    c->sens_ready = false;
-    c->march.U = c->march.dU = nullptr;
+    c->march.Up = c->march.dUp = nullptr;
+    c->xy.ready = false;
+    c->xy.Up = c->xy.dUp = nullptr;
+    c->sens_U = nullptr;
     c->visc.ready = false;
-    c->visc.Up = c->visc.dUp = nullptr;
+    c->visc.Ufp = c->visc.Up = c->visc.dUp = nullptr;
     c->timing = 0;
     c->tl_used = 0;
     if (launch_metric_tables(c) != OCFD_OK) { delete c; return OCFD_ECUDA; }
@@ -188,13 +177,21 @@ ocfd_status ocfd_fill_ghosts(ocfd_ctx *c, double *U) {
     return launch_fill_ghosts(c, U);
 }
 
-// rows a2-a7; rk_stage >= 0 additionally folds the RK3 stage update (a8) into the last kernel that touches dU
+// theta of U for the hybrid scheme: part of viscous pass 1 (which has staged everything the sensor needs), or the
+// stand-alone sensor kernel when there are no viscous terms
+static ocfd_status flux_and_sensor(ocfd_ctx *c, const double *U) {
+    const bool hybrid = c->p.scheme == OCFD_HYBRID;
+    if (!c->p.inviscid) return launch_viscous_flux(c, U, hybrid);
+    return hybrid ? launch_sensor(c, U) : OCFD_OK;
+}
+
+// rows a2-a7; rk_stage >= 0 additionally folds the RK3 stage update (a8) into the last kernel that touches dU.
+// Order: viscous pass 1 (+ sensor) first -- it depends on U only --, then the sweeps, then viscous pass 2 (+ RK3).
 static ocfd_status rhs_impl(ocfd_ctx *c, double *U, double *dU, int rk_stage, double dt) {
     ocfd_status st;
-    if ((st = launch_prim(c, U)) != OCFD_OK) return st;
-    if (c->p.scheme == OCFD_HYBRID && (st = launch_sensor(c, U)) != OCFD_OK) return st;
+    if ((st = flux_and_sensor(c, U)) != OCFD_OK) return st;
     if ((st = launch_inviscid(c, U, dU)) != OCFD_OK) return st;
-    if (!c->p.inviscid) return launch_viscous(c, dU, U, dt, rk_stage);
+    if (!c->p.inviscid) return launch_viscous_div(c, dU, U, dt, rk_stage);
     if (rk_stage >= 0) return launch_rk_update(c, c->Un, U, dU, dt, rk_stage);
     return OCFD_OK;
 }
@@ -243,8 +240,8 @@ ocfd_status ocfd_debug_sensor(ocfd_ctx *c, const double *U, double *theta, unsig
     // all-ones bytes are a NaN: what the sensor does not write (everything but the interior and the first ghost layer
     // of each face) comes back as NaN
     if (cudaMemsetAsync(c->theta, 0xff, c->g.np * sizeof(double), c->stream) != cudaSuccess) return OCFD_ECUDA;
-    if ((st = launch_prim(c, U)) != OCFD_OK) return st;
-    if ((st = launch_sensor(c, U)) != OCFD_OK) return st;
+    // the same kernel that computes theta inside ocfd_rhs / ocfd_rk3_step for this context
+    if ((st = c->p.inviscid ? launch_sensor(c, U) : launch_viscous_flux(c, U, true)) != OCFD_OK) return st;
     if (theta && cudaMemcpyAsync(theta, c->theta, c->g.np * sizeof(double), cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
         return OCFD_ECUDA;
     if (flag_xyz && (st = launch_flags(c, flag_xyz)) != OCFD_OK) return st;
@@ -275,7 +272,7 @@ ocfd_status ocfd_timing_read(ocfd_ctx *c, double *ms, long long *launches) {
 }
 
 const char *ocfd_kernel_name(int id) {
-    static const char *names[OCFD_NKERNELS] = {"ghost_fill", "primitives", "shock_sensor", "inviscid_x", "inviscid_y",
+    static const char *names[OCFD_NKERNELS] = {"ghost_fill", "shock_sensor", "inviscid_xy", "inviscid_x", "inviscid_y",
                                                "inviscid_z", "viscous_flux", "viscous_div", "rk3_update", "max_wavespeed"};
     return id >= 0 && id < OCFD_NKERNELS ? names[id] : "?";
 }
@@ -285,7 +282,7 @@ size_t ocfd_sizeof_params(void) { return sizeof(ocfd_params); }
 ocfd_status ocfd_set_tuning(ocfd_ctx *c, const char *key, int value) {
     if (!live(c)) return OCFD_ESTATE;
     if (!key || value < 0) return OCFD_EINVAL;
-    if (!strcmp(key, "x_sweep")) { if (value > 2) return OCFD_EINVAL; c->tune.x_sweep = value; pick_x_sweep(c); }
+    if (!strcmp(key, "xy_fused")) { if (value > 1) return OCFD_EINVAL; c->tune.xy_fused = value; }
     else if (!strcmp(key, "zchunk_flux")) c->tune.zchunk_f = value;
     else if (!strcmp(key, "zchunk_div")) c->tune.zchunk_d = value;
     else if (!strcmp(key, "zchunk_sensor")) c->tune.zchunk_s = value;

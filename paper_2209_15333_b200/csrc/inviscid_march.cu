@@ -1,12 +1,15 @@
-// Rows a4 + a5 for the y and z sweeps: Steger-Warming split (eq. 19-29), UD7 / WENO7 / WENO5
-// reconstruction (eq. 41) and the conservative flux difference, as a MARCHING kernel.
+// Rows a2 + a4 + a5 of ONE sweep direction: primitives from U, Steger-Warming split (eq. 19-29),
+// UD7 / WENO7 / WENO5 reconstruction (eq. 41) and the conservative flux difference, as a MARCHING
+// kernel.  It is the z sweep of every run (the x and y sweeps are fused in inviscid_xy.cu); its x and y instances
+// remain selectable (ocfd_set_tuning "xy_fused" = 0) as the unfused reference for A/B measurements.
 //
 // A CTA owns MAC = 32 pencils (32 consecutive x) of one cross index and walks along the sweep direction through all
 // nd + 8 padded rows in chunks of MR = 4 rows.  Every chunk:
-//   TMA      the state of the chunk (rho from U; u,v,w,c from the primitive fields; theta if hybrid) arrives in a ring
-//            of MNST = 3 stages that runs two chunks ahead of the arithmetic (one mbarrier per stage);
-//   phase A  one thread per point of the chunk: split fluxes f+-[5] -> shared memory.  Each point is split exactly
-//            once per sweep (no halo recomputation) and f+- never reach HBM (the paper materialises them, L549);
+//   TMA      the state of the chunk (the five conserved fields as ONE box; theta if hybrid) arrives in a ring of
+//            MNST = 3 stages that runs two chunks ahead of the arithmetic (one mbarrier per stage);
+//   phase A  one thread per point of the chunk: u, v, w, c from the conserved variables, then the split fluxes
+//            f+-[5] -> shared memory.  Each point is split exactly once per sweep (no halo recomputation) and neither
+//            the primitives nor f+- ever reach HBM (the paper materialises f+-, L549);
 //   phase B  one thread per (pencil, component): the 7-point windows of f+ and f- live in registers for the whole
 //            march, each new row costs two shared-memory loads; h_{i+1/2} is formed as soon as row i+4 has been
 //            pushed and -J (h_{i+1/2} - h_{i-1/2}) goes to an output tile in shared memory;
@@ -26,7 +29,7 @@ constexpr int MR = 4;               // rows per chunk
 constexpr int MNST = 3;             // input stages
 constexpr int MPTS = MAC * MR;      // points per chunk
 constexpr int MNT = 5 * MAC;        // threads: one walker per (pencil, component)
-constexpr int MSTG = 10 * MPTS;     // doubles per input stage: rho, u, v, w, c, theta, then k1, k2, k3, sigma (curvilinear)
+constexpr int MSTG = 10 * MPTS;     // doubles per input stage: U[5], theta, then k1, k2, k3, sigma (curvilinear)
 constexpr int MNJ = 4;              // slots of the J ring (curvilinear): J of chunk c is used while chunk c+1 is pushed
 constexpr size_t M_SMEM =
     sizeof(double) * (size_t)(MNST * MSTG + MNJ * MPTS + 10 * MPTS + 2 * 5 * MPTS) + 8 * MNST + 4 * MAC;
@@ -61,21 +64,6 @@ struct JRow {
     }
 };
 
-// h_{i+1/2} = recon(f+ window) + recon(mirrored f- window); out of line for the hybrid scheme (rare path, one copy)
-template <int SCHEME>
-__device__ __noinline__ double recon_pair_slow(int flag, double p0, double p1, double p2, double p3, double p4, double p5,
-                                               double p6, double m0, double m1, double m2, double m3, double m4, double m5,
-                                               double m6, double eps) {
-    return recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps) + recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
-}
-template <int SCHEME>
-__device__ __forceinline__ double recon_pair(int flag, double p0, double p1, double p2, double p3, double p4, double p5,
-                                             double p6, double m0, double m1, double m2, double m3, double m4, double m5,
-                                             double m6, double eps) {
-    if (SCHEME == OCFD_HYBRID) return recon_pair_slow<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, m0, m1, m2, m3, m4, m5, m6, eps);
-    return recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps) + recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
-}
-
 // KIND: grid kind, SCHEME: ocfd_scheme, DIR: 0 x, 1 y, 2 z.  grid = (tiles across, cross extent).
 // DIR 0: the 32 pencils are 32 consecutive y lines and a chunk is 4 x-points of each (boxes of 32-byte rows; the tensor
 // maps of the x sweep ask the L2 for 256-byte fills, so that the 8 chunks that share them find them there).  The
@@ -87,8 +75,8 @@ __device__ __forceinline__ double recon_pair(int flag, double p0, double p1, dou
 // gain nothing from the extra registers).
 template <int KIND, int SCHEME, int DIR>
 __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
-    k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_rho,
-                     const __grid_constant__ CUtensorMap tm_prim, const __grid_constant__ CUtensorMap tm_th,
+    k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_U,
+                     const __grid_constant__ CUtensorMap tm_th,
                      const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_met,
                      const __grid_constant__ CUtensorMap tm_metJ, const int mfull) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -121,8 +109,7 @@ __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
             tma::load4(dst + 6 * MPTS, &tm_met, &bars[s], c0, c1, m2, 0);
             tma::load4(sJ + (c % MNJ) * MPTS, &tm_metJ, &bars[s], c0, c1, m2, 4);
         }
-        tma::load4(dst, &tm_rho, &bars[s], c0, c1, c2, 0);
-        tma::load4(dst + MPTS, &tm_prim, &bars[s], c0, c1, c2, P_U);
+        tma::load4(dst, &tm_U, &bars[s], c0, c1, c2, 0);
         if (SCHEME == OCFD_HYBRID) tma::load4(dst + 5 * MPTS, &tm_th, &bars[s], c0, c1, c2, 0);
     };
     if (tid == 0) {
@@ -191,8 +178,10 @@ __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
         if (producer) {
             double *dst = sF + sfi;
             if (validA) {
-                sw_split_store<KIND, DIR>(gs, sU[tid], sU[MPTS + tid], sU[2 * MPTS + tid], sU[3 * MPTS + tid],
-                                          sU[4 * MPTS + tid], k1, k2, k3, sig, dst, MPTS);
+                double u, v, w, cc;
+                const double rho = sU[tid];
+                prim_from_cons(gs, rho, sU[MPTS + tid], sU[2 * MPTS + tid], sU[3 * MPTS + tid], sU[4 * MPTS + tid], u, v, w, cc);
+                sw_split_store<KIND, DIR>(gs, rho, u, v, w, cc, k1, k2, k3, sig, dst, MPTS);
             } else {
 #pragma unroll
                 for (int q = 0; q < 10; ++q) dst[q * MPTS] = 0.0;
@@ -317,8 +306,8 @@ ocfd_status launch_march(ocfd_ctx *c) {
     OCFD_T0(c, K_INV_X + DIR);
     const MarchMaps &M = c->march;
     const int mfull = DIR != 2 || g.msk != 0;
-    k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.rho[DIR], M.prim[DIR], M.th[DIR],
-                                                                        M.out[DIR], M.met[DIR], M.metJ[DIR], mfull);
+    k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.U[DIR], M.th[DIR], M.out[DIR],
+                                                                        M.met[DIR], M.metJ[DIR], mfull);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
@@ -342,11 +331,11 @@ ocfd_status launch_march_kind(ocfd_ctx *c, int dir) {
 bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
     const GridDesc &g = c->g;
     MarchMaps &M = c->march;
-    const long long full1[4] = {g.nxp, g.nyp, g.nzp, 1}, full6[4] = {g.nxp, g.nyp, g.nzp, P_NF};
+    const long long full1[4] = {g.nxp, g.nyp, g.nzp, 1}, full5[4] = {g.nxp, g.nyp, g.nzp, 5};
     const long long inner[4] = {g.nx, g.ny, g.nz, 5};
     for (int d = 0; d < 3; ++d) {
         const int bx = d == 0 ? MR : MAC, by = d == 0 ? MAC : d == 1 ? MR : 1, bz = d == 2 ? MR : 1;
-        const int b1[4] = {bx, by, bz, 1}, b4[4] = {bx, by, bz, 4}, bo[4] = {bx, by, bz, 5};
+        const int b1[4] = {bx, by, bz, 1}, bo[4] = {bx, by, bz, 5};
         if (!M.ready) {
             if (g.kind == OCFD_GRID_CURVILINEAR) {
                 // the derived metric table of this direction: [5][planes][nyp][nxp], one plane if z-extruded
@@ -358,17 +347,16 @@ bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
             } else {   // unused, but the kernel takes the parameters
                 M.met[d] = M.metJ[d] = CUtensorMap();
             }
-            if (!ocfd_tma_encode(&M.prim[d], c->prim, full6, g.sy, g.sz, g.np, b4, d == 0)) return false;
             if (!ocfd_tma_encode(&M.th[d], c->theta, full1, g.sy, g.sz, g.np, b1, d == 0)) return false;
         }
-        if (M.U != U && !ocfd_tma_encode(&M.rho[d], U, full1, g.sy, g.sz, g.np, b1, d == 0)) return false;
-        if (M.dU != dU &&
+        if (M.Up != U && !ocfd_tma_encode(&M.U[d], U, full5, g.sy, g.sz, g.np, bo, d == 0)) return false;
+        if (M.dUp != dU &&
             !ocfd_tma_encode(&M.out[d], dU + (long long)OCFD_NG * (g.sz + g.sy + 1), inner, g.sy, g.sz, g.np, bo))
             return false;
     }
     M.ready = true;
-    M.U = U;
-    M.dU = dU;
+    M.Up = U;
+    M.dUp = dU;
     return true;
 }
 

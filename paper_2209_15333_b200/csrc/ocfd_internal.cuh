@@ -47,34 +47,41 @@ struct GasDesc {
     double weno_eps, sw_eps, theta1, theta2;
 };
 
-// kernel classes, for ocfd_timing_read / ocfd_kernel_name
-enum { K_GHOST = 0, K_PRIM, K_SENSOR, K_INV_X, K_INV_Y, K_INV_Z, K_VISC_FLUX, K_VISC_DIV, K_RK, K_WAVE, K_COUNT };
+// kernel classes, for ocfd_timing_read / ocfd_kernel_name (K_INV_X + d = the sweep of direction d as its own launch)
+enum { K_GHOST = 0, K_SENSOR, K_INV_XY, K_INV_X, K_INV_Y, K_INV_Z, K_VISC_FLUX, K_VISC_DIV, K_RK, K_WAVE, K_COUNT };
 static_assert(K_COUNT == OCFD_NKERNELS, "kernel class count");
 
 struct TimedLaunch { cudaEvent_t a, b; int id; };
 
-// TMA tensor maps of the inviscid sweeps (per direction), re-encoded only when the caller's U / dU pointers change
+// TMA tensor maps of the tile sweeps (characteristic variables; per direction), re-encoded only when the caller's
+// U / dU pointers change
 struct InvMaps {
-    const double *U, *dU;
+    const double *Up, *dUp;
     bool ready;
-    CUtensorMap rho[3], prim[3], th[3], out[3];
+    CUtensorMap U[3], th[3], out[3];
 };
 // ... of the marching sweeps (inviscid_march.cu), same roles, other box shapes
 struct MarchMaps {
-    const double *U, *dU;
+    const double *Up, *dUp;
     bool ready;
-    CUtensorMap rho[3], prim[3], th[3], out[3], met[3], metJ[3];
+    CUtensorMap U[3], th[3], out[3], met[3], metJ[3];
+};
+// ... of the fused x-y sweep (inviscid_xy.cu)
+struct XYMaps {
+    const double *Up, *dUp;
+    bool ready;
+    CUtensorMap U, th, out;
 };
 // ... and of the two viscous passes
 struct ViscMaps {
-    const double *Up, *dUp;
+    const double *Ufp, *Up, *dUp;
     bool ready;
-    CUtensorMap prim, F, G, H, dU, U, Un;
+    CUtensorMap Uf, F, G, H, dU, U, Un;
 };
 
 // Tuning knobs of one context (ocfd_set_tuning): launch-shape choices that change no result beyond round-off.
 struct Tuning {
-    int x_sweep;     // 0 automatic, 1 tile kernel, 2 marching kernel
+    int xy_fused;    // 1 (default): x and y sweeps in one kernel; 0: one marching launch per direction (A/B reference)
     int zchunk_f;    // planes per CTA of viscous pass 1 (0 automatic)
     int zchunk_d;    // ... of viscous pass 2
     int zchunk_s;    // ... of the shock sensor
@@ -87,12 +94,10 @@ struct ocfd_ctx {
     GasDesc gas;
     cudaStream_t stream;
     int visc_order;  // 6 or 8 (ocfd_params.visc_order, 0 -> 6)
-    int x_tile;      // x sweep by the tile kernel of inviscid.cu (1: default for WENO7 / WENO5) or the marching kernel (0: UD7, hybrid)
     int nsm;         // SM count of the device (persistent kernels launch a multiple of it)
     Tuning tune;
     std::vector<const void *> smem_optin;   // kernels whose dynamic shared-memory limit has been raised in this context
     // workspace carve-up (device pointers)
-    double *prim;    // [6][np]: T u v w c p
     double *theta;   // [np]
     double *Fv;      // [12][np]
     double *Un;      // [5][np]
@@ -102,8 +107,9 @@ struct ocfd_ctx {
     unsigned char *flags;  // [3][np] bytes (debug only)
     InvMaps inv;
     MarchMaps march;
-    CUtensorMap sens_map;   // p with a 1-point x-y halo (shock sensor)
-    bool sens_ready;
+    XYMaps xy;
+    CUtensorMap sens_map;   // U with a 1-point x-y halo (stand-alone shock sensor)
+    const double *sens_U;
     ViscMaps visc;
     long long launches;
     // optional per-launch timing with CUDA events on the launch stream (ocfd_timing)
@@ -130,10 +136,6 @@ inline void ocfd_t1(ocfd_ctx *c) {
     c->tl_used++;
 }
 #define OCFD_T0(ctx, id) ocfd_t0((ctx), (id))
-
-// prim field order
-// (T first and c after w: the viscous kernels fetch fields 0..3 = T,u,v,w, the inviscid sweeps 1..4 = u,v,w,c as one box)
-enum { P_T = 0, P_U = 1, P_V = 2, P_W = 3, P_C = 4, P_P = 5, P_NF = 6 };
 
 // ---------------------------------------------------------------- metric access
 // padded linear index of (ip,jp,kp)
@@ -203,12 +205,13 @@ __device__ __forceinline__ void met_ksJ(const GridDesc &g, int ip, int jp, int k
 // ---------------------------------------------------------------- kernel launchers (host side)
 ocfd_status launch_metric_tables(ocfd_ctx *c);
 ocfd_status launch_fill_ghosts(ocfd_ctx *c, double *U);
-ocfd_status launch_prim(ocfd_ctx *c, const double *U);
 ocfd_status launch_sensor(ocfd_ctx *c, const double *U);
 ocfd_status launch_flags(ocfd_ctx *c, unsigned char *flags);
 ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU);
-ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int dir);  // dir = 1 (y) or 2 (z)
-ocfd_status launch_viscous(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage);
+ocfd_status launch_inviscid_xy(ocfd_ctx *c, const double *U, double *dU);
+ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int dir);
+ocfd_status launch_viscous_flux(ocfd_ctx *c, const double *U, bool sensor);
+ocfd_status launch_viscous_div(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage);
 ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage);
 ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
 

@@ -1,4 +1,4 @@
-// Rows a2 (primitives), a3 (shock sensor) and a9 (max wavespeed).
+// Rows a3 (shock sensor, stand-alone form) and a9 (max wavespeed); row a2 (primitives) lives inside its consumers.
 #include "ocfd_internal.cuh"
 #include "schemes.cuh"
 #include "tma.cuh"
@@ -6,63 +6,33 @@
 
 namespace {
 
-// a2: u,v,w,T,c,p at every padded point (eq. 8 as corrected, eq. 16).  Edge / corner ghosts
-// hold whatever the caller left there; their primitives are computed but never read.
-__global__ void __launch_bounds__(256) k_prim(long long np, GasDesc gs, const double *__restrict__ U,
-                                              double *__restrict__ prim) {
-    // two consecutive points per thread as 16-byte accesses (np is even: nx is), two pairs in flight per thread
-    const long long npair = np >> 1, stride = (long long)gridDim.x * blockDim.x;
-    const double2 *U2 = reinterpret_cast<const double2 *>(U);
-    double2 *P2 = reinterpret_cast<double2 *>(prim);
-    for (long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x; id < npair; id += 2 * stride) {
-        double2 q[2][5];
-        bool ok[2];
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            ok[e] = id + e * stride < npair;
-            if (ok[e]) {
-#pragma unroll
-                for (int m = 0; m < 5; ++m) q[e][m] = __ldcs(U2 + m * npair + id + e * stride);
-            }
-        }
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            if (!ok[e]) continue;
-            double2 u, v, w, p, T, c;
-            // true divisions (not a reciprocal multiply): this kernel is HBM-bound, and the pressure that feeds
-            // the shock-sensor decisions then rounds exactly as the definition does
-            u.x = q[e][1].x / q[e][0].x; v.x = q[e][2].x / q[e][0].x; w.x = q[e][3].x / q[e][0].x;
-            u.y = q[e][1].y / q[e][0].y; v.y = q[e][2].y / q[e][0].y; w.y = q[e][3].y / q[e][0].y;
-            p.x = gs.gm1 * (q[e][4].x - 0.5 * q[e][0].x * (u.x * u.x + v.x * v.x + w.x * w.x));
-            p.y = gs.gm1 * (q[e][4].y - 0.5 * q[e][0].y * (u.y * u.y + v.y * v.y + w.y * w.y));
-            T.x = gs.gM2 * p.x / q[e][0].x; T.y = gs.gM2 * p.y / q[e][0].y;
-            c.x = sqrt(T.x) * gs.invMa; c.y = sqrt(T.y) * gs.invMa;
-            const long long o = id + e * stride;
-            P2[P_U * npair + o] = u;
-            P2[P_V * npair + o] = v;
-            P2[P_W * npair + o] = w;
-            P2[P_T * npair + o] = T;
-            P2[P_C * npair + o] = c;
-            P2[P_P * npair + o] = p;
-        }
-    }
-}
-
-// a3: theta = phi_i + phi_j + phi_k at interior points (eq. 42, R-11) and its first ghost layer (R-12).
+// a3 (stand-alone form, for runs without viscous terms; with them the sensor is part of viscous pass 1, viscous.cu):
+// theta = phi_i + phi_j + phi_k at interior points (eq. 42, R-11) and its first ghost layer (R-12).
 // phi_d = |p_- - 2 p_0 + p_+| / (p_- + 2 p_0 + p_+); the three quotients share one division:
 // theta = (n_i d_j d_k + n_j d_i d_k + n_k d_i d_j) / (d_i d_j d_k).
 //
-// 2.5-D marching kernel: a CTA owns an ST x SY tile in x-y and walks along z; every plane of p (with its 1-point x-y
-// halo) is fetched once by a TMA box load into a ring of shared-memory stages that runs ahead of the arithmetic, so
-// p is read once from HBM (8 B/point) and theta written once (8 B/point).
+// 2.5-D marching kernel: a CTA owns an ST x SY tile in x-y and walks along z; every plane of U (with its 1-point x-y
+// halo) is fetched once by a TMA box load into a ring of shared-memory stages that runs ahead of the arithmetic; the
+// CTA turns each landed plane into p in place (row a2: no primitive field exists in HBM), so U is read once from HBM
+// (40 B/point) and theta written once (8 B/point).
 constexpr int ST = 32, SY = 8, SNT = ST * SY;
 constexpr int SBX = ST + 4, SBY = SY + 2;          // box with halo; 2 wider in x on each side: a box of doubles starts at an even x
-constexpr int S_NST = 6;                           // ring: planes k-1, k, k+1 live, three more in flight
-constexpr int S_STAGE = (SBX * SBY * 8 + 127) / 128 * 128 / 8;   // doubles per stage, 128-byte aligned
+constexpr int S_FLD = SBX * SBY;                   // doubles per staged field
+constexpr int S_NST = 4;                           // ring: planes k, k+1 live, k+2 being converted, one more in flight
+constexpr int S_STAGE = (5 * S_FLD * 8 + 127) / 128 * 128 / 8;   // doubles per stage, 128-byte aligned
 constexpr size_t S_SMEM = sizeof(double) * S_NST * S_STAGE + 8 * S_NST;
 
-__global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, const __grid_constant__ CUtensorMap tm_p,
-                                                double *__restrict__ theta, int zchunk) {
+// p of the points of one staged plane of U, left in the slot of rho
+__device__ __forceinline__ void pressure_plane(const GasDesc &gs, double *st, int tid) {
+    for (int q = tid; q < S_FLD; q += SNT) {
+        const double rho = st[q], ir = fast_rcp_pos(rho);
+        const double u = st[S_FLD + q] * ir, v = st[2 * S_FLD + q] * ir, w = st[3 * S_FLD + q] * ir;
+        st[q] = gs.gm1 * (st[4 * S_FLD + q] - 0.5 * rho * (u * u + v * v + w * w));
+    }
+}
+
+__global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, GasDesc gs, const __grid_constant__ CUtensorMap tm_U,
+                                                const double *__restrict__ U, double *__restrict__ theta, int zchunk) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + S_NST * S_STAGE);
@@ -71,29 +41,37 @@ __global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, const __grid_constan
     const int i = i0 + tx, j = j0 + ty;
     const bool own = i < g.nx && j < g.ny;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
-    // plane q of the march = interior plane k0 - 1 + q; stage q % S_NST
-    const int nplanes = k1 - k0 + 2;
-    auto issue = [&](int q) {
-        const int s = q % S_NST;
-        tma::mbar_expect_tx(&bars[s], SBX * SBY * 8);
-        tma::load4(ring + s * S_STAGE, &tm_p, &bars[s], i0 + OCFD_NG - 2, j0 + OCFD_NG - 1, k0 - 1 + q + OCFD_NG, P_P);
+    const int last = k1;   // last plane needed (k1 - 1 + 1)
+    auto issue = [&](int plane) {   // interior plane index -> stage (plane - k0) % S_NST
+        const int s = (plane - k0) % S_NST;
+        tma::mbar_expect_tx(&bars[s], 5 * S_FLD * 8);
+        tma::load4(ring + s * S_STAGE, &tm_U, &bars[s], i0 + OCFD_NG - 2, j0 + OCFD_NG - 1, plane + OCFD_NG, 0);
     };
     if (tid == 0) {
         for (int s = 0; s < S_NST; ++s) tma::mbar_init(&bars[s], 1);
         tma::fence_barrier_init();
-        for (int q = 0; q < S_NST && q < nplanes; ++q) issue(q);
+        for (int q = 0; q < S_NST; ++q)
+            if (k0 + q <= last) issue(k0 + q);
+    }
+    // p of plane k0-1 at this thread's column, straight from global memory
+    double pm;
+    {
+        const int ipc = min(i, g.nx - 1) + OCFD_NG, jpc = min(j, g.ny - 1) + OCFD_NG;
+        const long long id = (long long)(k0 - 1 + OCFD_NG) * g.sz + (long long)jpc * g.sy + ipc;
+        const double rho = __ldg(U + id), ir = fast_rcp_pos(rho);
+        const double u = __ldg(U + g.np + id) * ir, v = __ldg(U + 2 * g.np + id) * ir, w = __ldg(U + 3 * g.np + id) * ir;
+        pm = gs.gm1 * (__ldg(U + 4 * g.np + id) - 0.5 * rho * (u * u + v * v + w * w));
+    }
+    __syncthreads();   // barriers initialised
+    for (int q = 0; q < 2; ++q) {   // planes k0, k0+1 (both exist: k0+1 <= k1)
+        tma::mbar_wait(&bars[q], 0);
+        pressure_plane(gs, ring + q * S_STAGE, tid);
     }
     __syncthreads();
     const int ctr = (ty + 1) * SBX + tx + 2;
-    tma::mbar_wait(&bars[0], 0);
-    tma::mbar_wait(&bars[1], 0);
-    double pm = ring[ctr], p0 = ring[S_STAGE + ctr];
     for (int k = k0; k < k1; ++k) {
-        const int q = k - k0 + 2;   // plane k+1
-        const int s = q % S_NST;
-        tma::mbar_wait(&bars[s], (q / S_NST) & 1);
-        const double pp = ring[s * S_STAGE + ctr];
-        const double *c = ring + ((q - 1) % S_NST) * S_STAGE + ctr;
+        const double *c = ring + ((k - k0) % S_NST) * S_STAGE + ctr;
+        const double p0 = c[0], pp = ring[((k + 1 - k0) % S_NST) * S_STAGE + ctr];
         if (own) {
             const double t0 = p0 + p0;
             const double ni = fabs(t0 - c[-1] - c[1]), di = t0 + c[-1] + c[1];
@@ -114,9 +92,13 @@ __global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, const __grid_constan
             }
         }
         pm = p0;
-        p0 = pp;
-        __syncthreads();   // everyone is done with plane k-1: its stage can be refilled
-        if (tid == 0 && q - 2 + S_NST < nplanes) issue(q - 2 + S_NST);
+        if (k + 2 <= last) {   // the plane after next: turn it into p now, one barrier publishes it and frees plane k
+            const int sc = (k + 2 - k0) % S_NST;
+            tma::mbar_wait(&bars[sc], ((k + 2 - k0) / S_NST) & 1);
+            pressure_plane(gs, ring + sc * S_STAGE, tid);
+        }
+        __syncthreads();
+        if (tid == 0 && k + S_NST <= last) issue(k + S_NST);
     }
 }
 
@@ -182,37 +164,24 @@ __global__ void __launch_bounds__(256) k_wavespeed(GridDesc g, GasDesc gs, const
 
 }  // namespace
 
-ocfd_status launch_prim(ocfd_ctx *c, const double *U) {
-    long long np = c->g.np;
-    int blocks = (int)((np / 4 + 255) / 256);   // a thread takes two pairs of points per pass
-    if (blocks < 1) blocks = 1;
-    if (blocks > c->nsm * 16) blocks = c->nsm * 16;
-    OCFD_T0(c, K_PRIM);
-    k_prim<<<blocks, 256, 0, c->stream>>>(np, c->gas, U, c->prim);
-    OCFD_CHECK_LAUNCH(c);
-    return OCFD_OK;
-}
-
 ocfd_status launch_sensor(ocfd_ctx *c, const double *U) {
-    (void)U;
     const GridDesc &g = c->g;
-    if (!c->sens_ready) {
-        const long long d6[4] = {g.nxp, g.nyp, g.nzp, P_NF};
-        const int bx[4] = {SBX, SBY, 1, 1};
-        if (!ocfd_tma_encode(&c->sens_map, c->prim, d6, g.sy, g.sz, g.np, bx)) return OCFD_ECUDA;
-        if (cudaFuncSetAttribute(k_sensor, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S_SMEM) != cudaSuccess)
-            return OCFD_ECUDA;
-        c->sens_ready = true;
+    if (c->sens_U != U) {
+        const long long d5[4] = {g.nxp, g.nyp, g.nzp, 5};
+        const int bx[4] = {SBX, SBY, 1, 5};
+        if (!ocfd_tma_encode(&c->sens_map, U, d5, g.sy, g.sz, g.np, bx)) return OCFD_ECUDA;
+        c->sens_U = U;
     }
-    // enough blocks to fill the SMs a few times over, chunks long enough that the two prologue planes stay cheap
+    if (!ocfd_smem_optin(c, (const void *)k_sensor, S_SMEM)) return OCFD_ECUDA;
+    // enough blocks to fill the SMs a few times over, chunks long enough that the prologue planes stay cheap
     const long long tiles = (long long)((g.nx + ST - 1) / ST) * ((g.ny + SY - 1) / SY);
     int zc = g.nz;
     while (zc > 32 && tiles * ((g.nz + zc - 1) / zc) < c->nsm * 16) zc = (zc + 1) / 2;
-    if (zc > 64) zc = 64;   // short marches keep halo-sharing tiles close in z (as in the viscous kernels; 0.64 -> 0.59 ms)
+    if (zc > 64) zc = 64;   // short marches keep halo-sharing tiles close in z (as in the viscous kernels)
     if (c->tune.zchunk_s >= 8) zc = c->tune.zchunk_s < g.nz ? c->tune.zchunk_s : g.nz;
     dim3 blk(ST, SY, 1), grd((g.nx + ST - 1) / ST, (g.ny + SY - 1) / SY, (g.nz + zc - 1) / zc);
     OCFD_T0(c, K_SENSOR);
-    k_sensor<<<grd, blk, S_SMEM, c->stream>>>(g, c->sens_map, c->theta, zc);
+    k_sensor<<<grd, blk, S_SMEM, c->stream>>>(g, c->gas, c->sens_map, U, c->theta, zc);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }

