@@ -141,9 +141,10 @@ ocfd_status ocfd_max_wavespeed(ocfd_ctx *ctx, const double *U, double *host_out)
 ocfd_status ocfd_debug_sensor(ocfd_ctx *ctx, const double *U, double *theta, unsigned char *flag_xyz);
 
 /* Launch-shape knobs of one context, for A/B measurements; they change no result beyond round-off.  Keys:
- * "xy_fused" (1, default: the x and y sweeps run as one kernel; 0: one marching launch per direction, the unfused
- * reference), "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a CTA of the viscous passes / the stand-alone sensor
- * marches; 0 automatic, else >= 8).  Unknown key or negative value: OCFD_EINVAL. */
+ * "xy_fused" (0, default: one marching launch per sweep direction; 1: the x and y sweeps run as one kernel, an
+ * experiment that is slower on every measured workload), "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a CTA of
+ * the viscous passes / the stand-alone sensor marches; 0 automatic, else >= 8), "march_seg" (segments a pencil of the
+ * marching sweeps is cut into; 0 automatic).  Unknown key or negative value: OCFD_EINVAL. */
 ocfd_status ocfd_set_tuning(ocfd_ctx *ctx, const char *key, int value);
 
 /* sizeof(ocfd_params) as compiled, so that a foreign-language mirror of the struct can check itself. */

@@ -65,6 +65,7 @@ Carve carve(const ocfd_params *p) {
     if (p->grid_kind == OCFD_GRID_CURVILINEAR) {
         const size_t planes = p->metric_plane_stride ? (size_t)(p->nz + 8) : 1;
         off += align_up(15 * planes * (size_t)(p->nx + 8) * (p->ny + 8) * sizeof(double), 256);
+        off += align_up(5 * planes * (size_t)(p->nx + 8) * (size_t)((p->ny + 9) & ~1) * sizeof(double), 256);  // atabT
     } else if (p->grid_kind == OCFD_GRID_STRETCHED) {
         off += align_up((size_t)(p->nx + p->ny + p->nz + 24) * sizeof(double), 256);
     }
@@ -102,7 +103,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->stream = (cudaStream_t)p->stream;
     c->nsm = nsm;
     c->tune = Tuning();
-    c->tune.xy_fused = 1;
+    c->tune.xy_fused = 0;
     c->visc_order = p->visc_order == 8 ? 8 : 6;
     GridDesc &g = c->g;
     g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
@@ -137,6 +138,7 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->mtab = (double *)(w + cv.mtab);
     for (int d = 0; d < 3; ++d) { g.atab[d] = nullptr; g.rmet[d] = nullptr; g.ua[d] = 0.0; }
     g.atab_fs = 0;
+    g.atabT = nullptr; g.atabT_fs = 0; g.nypT = (g.nyp + 1) & ~1;
     if (p->grid_kind == OCFD_GRID_UNIFORM) {
         g.ua[0] = g.ux / g.uJ; g.ua[1] = g.uy / g.uJ; g.ua[2] = g.uz / g.uJ;
     } else if (p->grid_kind == OCFD_GRID_STRETCHED) {
@@ -144,6 +146,8 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     } else {
         g.atab_fs = (g.msk ? (long long)g.nzp : 1ll) * g.sz;
         for (int d = 0; d < 3; ++d) g.atab[d] = c->mtab + 5 * d * g.atab_fs;
+        g.atabT_fs = (g.msk ? (long long)g.nzp : 1ll) * g.nxp * g.nypT;
+        g.atabT = c->mtab + (align_up(15 * (size_t)g.atab_fs * sizeof(double), 256) / sizeof(double));
     }
     c->flags = nullptr;
     c->launches = 0;
@@ -286,6 +290,7 @@ ocfd_status ocfd_set_tuning(ocfd_ctx *c, const char *key, int value) {
     else if (!strcmp(key, "zchunk_flux")) c->tune.zchunk_f = value;
     else if (!strcmp(key, "zchunk_div")) c->tune.zchunk_d = value;
     else if (!strcmp(key, "zchunk_sensor")) c->tune.zchunk_s = value;
+    else if (!strcmp(key, "march_seg")) c->tune.march_seg = value;
     else return OCFD_EINVAL;
     return OCFD_OK;
 }

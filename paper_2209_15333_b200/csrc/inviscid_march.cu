@@ -31,8 +31,9 @@ constexpr int MPTS = MAC * MR;      // points per chunk
 constexpr int MNT = 5 * MAC;        // threads: one walker per (pencil, component)
 constexpr int MSTG = 10 * MPTS;     // doubles per input stage: U[5], theta, then k1, k2, k3, sigma (curvilinear)
 constexpr int MNJ = 4;              // slots of the J ring (curvilinear): J of chunk c is used while chunk c+1 is pushed
+constexpr int MTMA = MPTS;          // the thread that issues every TMA operation: lane 0 of the warp without phase-A work
 constexpr size_t M_SMEM =
-    sizeof(double) * (size_t)(MNST * MSTG + MNJ * MPTS + 10 * MPTS + 2 * 5 * MPTS) + 8 * MNST + 4 * MAC;
+    sizeof(double) * (size_t)(MNST * MSTG + MNJ * MPTS + 2 * 10 * MPTS + 2 * 5 * MPTS) + 8 * MNST + 2 * 4 * MAC;
 static_assert(MPTS <= MNT && (MPTS * 8) % 128 == 0, "chunk shape");
 
 // J along one pencil of the sweep: at(g, i0, e) = J at padded row i0 + e
@@ -70,32 +71,35 @@ struct JRow {
 // shared arrays keep the box order (x fastest), the split fluxes are stored with an XOR swizzle of the pencil index so
 // that both the point-wise phase and the walkers are free of bank conflicts, and the output tile is written as two
 // 16-byte stores per walker and leaves by a TMA store (the x sweep writes dU, y and z accumulate).
-// Occupancy: 4 CTAs per SM (96 registers) except for the hybrid scheme, whose three code paths need 128 registers to keep
-// the unrolled linear path free of spills (measured: 3.8 ms against 4.5 ms per sweep on config 5; the WENO7 kernels
-// gain nothing from the extra registers).
+// Occupancy: 3 CTAs per SM (128 registers, 65 KB of shared memory each): the hybrid scheme's three code paths need the
+// 128 registers to keep the unrolled linear path free of spills (measured: 3.8 ms against 4.5 ms per sweep on config 5).
 template <int KIND, int SCHEME, int DIR>
-__global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
+__global__ void __launch_bounds__(MNT, 3)
     k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_U,
                      const __grid_constant__ CUtensorMap tm_th,
                      const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_met,
-                     const __grid_constant__ CUtensorMap tm_metJ, const int mfull) {
+                     const __grid_constant__ CUtensorMap tm_metJ, const int mfull, const int seglen) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *sIn = reinterpret_cast<double *>(smem_raw);   // [MNST][10][MR][MAC]
     double *sJ = sIn + MNST * MSTG;                       // [MNJ][MR][MAC]
-    double *sF = sJ + MNJ * MPTS;                         // [10][MR][MAC]: f+ (0..4), f- (5..9) of the current chunk
-    double *sO = sF + 10 * MPTS;                          // [2][5][MR][MAC] output tiles
+    double *sF = sJ + MNJ * MPTS;                         // [2][10][MR][MAC]: f+ (0..4), f- (5..9) of chunk c in buffer c % 2
+    double *sO = sF + 2 * 10 * MPTS;                      // [2][5][MR][MAC] output tiles
     uint64_t *bars = reinterpret_cast<uint64_t *>(sO + 2 * 5 * MPTS);
-    unsigned char *sFl = reinterpret_cast<unsigned char *>(bars + MNST);   // [MAC][MR] scheme flags pf of the chunk
+    unsigned char *sFl = reinterpret_cast<unsigned char *>(bars + MNST);   // [2][MAC][MR] scheme flags pf of chunk c % 2
 
     const int tid = threadIdx.x;
     const int a0 = blockIdx.x * MAC, cross = blockIdx.y;
     const int nd = DIR == 0 ? g.nx : DIR == 1 ? g.ny : g.nz;
     const int nap = DIR == 0 ? g.nyp : g.nxp;   // padded extent across
     const int ndp = nd + 2 * OCFD_NG;
-    const int nch = (ndp + MR - 1) / MR;
+    // blockIdx.z = segment of the march: interior rows [o0, o1) (seglen is a multiple of MR; short segments keep the
+    // CTAs short, which evens out the end of the launch when the cross-section gives few CTAs).  A segment stages the
+    // padded rows o0 .. o1 + 7, i.e. the chunks [cbeg, cend); every per-chunk slot below is indexed by lc = c - cbeg.
+    const int o0 = blockIdx.z * seglen, o1 = min(o0 + seglen, nd);
+    const int cbeg = o0 / MR, cend = (o1 + 2 * OCFD_NG + MR - 1) / MR, nch = cend - cbeg;
 
-    auto issue = [&](int c) {   // one thread: boxes of chunk c (padded rows MR*c ..) towards stage c % MNST
-        const int s = c % MNST;
+    auto issue = [&](int lc) {   // one thread: boxes of chunk c (padded rows MR*c ..) towards stage lc % MNST
+        const int c = cbeg + lc, s = lc % MNST;
         double *dst = sIn + s * MSTG;
         const int c0 = DIR == 0 ? MR * c : OCFD_NG + a0;
         const int c1 = DIR == 0 ? OCFD_NG + a0 : DIR == 1 ? MR * c : OCFD_NG + cross;
@@ -106,18 +110,20 @@ __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
         tma::mbar_expect_tx(&bars[s], (SCHEME == OCFD_HYBRID ? 6 : 5) * MPTS * 8 + mbytes);
         if (KIND == OCFD_GRID_CURVILINEAR) {
             const int m2 = DIR == 2 ? (mfull ? MR * c : 0) : (g.msk ? OCFD_NG + cross : 0);
-            tma::load4(dst + 6 * MPTS, &tm_met, &bars[s], c0, c1, m2, 0);
-            tma::load4(sJ + (c % MNJ) * MPTS, &tm_metJ, &bars[s], c0, c1, m2, 4);
+            // (x sweep: the copy of the table with y contiguous, so the box is [4 x][32 lines])
+            tma::load4(dst + 6 * MPTS, &tm_met, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 0);
+            tma::load4(sJ + (lc % MNJ) * MPTS, &tm_metJ, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 4);
         }
         tma::load4(dst, &tm_U, &bars[s], c0, c1, c2, 0);
         if (SCHEME == OCFD_HYBRID) tma::load4(dst + 5 * MPTS, &tm_th, &bars[s], c0, c1, c2, 0);
     };
-    if (tid == 0) {
+    if (tid == MTMA) {
 #pragma unroll
         for (int q = 0; q < MNST; ++q) tma::mbar_init(&bars[q], 1);
         tma::fence_barrier_init();
         issue(0);
         if (nch > 1) issue(1);
+        if (nch > 2) issue(2);
     }
 
     // phase A role: point (row pr, pencil pa) of every chunk; walker role: pencil wa, component wm
@@ -139,77 +145,74 @@ __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
     unsigned pprev = 0;     // packed scheme flags pf(r) of the previous chunk's rows, 2 bits per row (hybrid)
     __syncthreads();        // barriers initialised before anyone polls them
 
-    // one chunk; PH = c % 2 fixes the ring slots at compile time
-    auto chunk = [&](const int c, auto ph) {
-        constexpr int PH = decltype(ph)::value;
-        const int s = c % MNST;
+    // ---- phase A of chunk c: split fluxes of the chunk's points -> sF[c % 2]; pf(r) = scheme flag of the interface
+    // between rows r-1 and r -> sFl[c % 2]
+    auto phaseA = [&](const int lc) {
+        const int s = lc % MNST;
         const double *sU = sIn + s * MSTG;
-        const int r0 = MR * c;   // first padded row of the chunk
-
-        // metric data, fetched while the boxes are in flight: k, sigma of this thread's point (phase A) ...
-        double k1 = 0.0, k2 = 0.0, k3 = 0.0, sig = 1.0, Jdead;
-        const int rowA = r0 + pr;
+        const int rowA = MR * (cbeg + lc) + pr;
         const bool validA = producer && x_ok && rowA < ndp;
+        // metric data of this thread's point, fetched while the boxes are in flight
+        double k1 = 0.0, k2 = 0.0, k3 = 0.0, sig = 1.0, Jdead;
         if (KIND != OCFD_GRID_CURVILINEAR && validA)
             met_ksJ<KIND, DIR>(g, DIR == 0 ? rowA : apA, DIR == 0 ? apA : DIR == 1 ? rowA : OCFD_NG + cross,
                                DIR == 2 ? rowA : OCFD_NG + cross, k1, k2, k3, sig, Jdead);
-        // ... and J of the four points this walker completes in this chunk (padded rows r0-4 .. r0-1; the first
-        // chunk completes nothing that is kept)
+        tma::mbar_wait(&bars[s], (lc / MNST) & 1);   // every thread: the walkers read J of this stage one chunk later
+        if (!producer) return;
+        if (KIND == OCFD_GRID_CURVILINEAR && validA) {
+            // the metric box lands densely: field stride = its own row count x MAC
+            const int mi = DIR == 0 ? pr * MAC + pa : mfull ? tid : pa, mfs = mfull ? MPTS : MAC;
+            const double *mp = sU + 6 * MPTS + mi;
+            k1 = mp[0]; k2 = mp[mfs]; k3 = mp[2 * mfs]; sig = mp[3 * mfs];
+        }
+        double *dst = sF + (lc & 1) * 10 * MPTS + sfi;
+        if (validA) {
+            double u, v, w, cc;
+            const double rho = sU[tid];
+            prim_from_cons(gs, rho, sU[MPTS + tid], sU[2 * MPTS + tid], sU[3 * MPTS + tid], sU[4 * MPTS + tid], u, v, w, cc);
+            sw_split_store<KIND, DIR>(gs, rho, u, v, w, cc, k1, k2, k3, sig, dst, MPTS);
+        } else {
+#pragma unroll
+            for (int q = 0; q < 10; ++q) dst[q * MPTS] = 0.0;
+        }
+        if (SCHEME == OCFD_HYBRID) {
+            unsigned char f = 0;
+            // interfaces -1/2 .. nd-1/2 (eq. 42, R-12) of live pencils: a pencil past the last interior line would read
+            // theta from ghost rows nobody wrote, and one lane on the non-linear path costs its whole warp that path
+            if (x_ok && rowA >= OCFD_NG && rowA <= nd + OCFD_NG) {
+                const double *thp =
+                    pr > 0 ? sU + 5 * MPTS + tid - (DIR == 0 ? 1 : MAC)
+                           : sIn + ((lc + MNST - 1) % MNST) * MSTG + 5 * MPTS + (DIR == 0 ? tid + MR - 1 : (MR - 1) * MAC + pa);
+                f = (unsigned char)iface_flag(gs, *thp, sU[5 * MPTS + tid]);
+            }
+            sFl[(lc & 1) * 4 * MAC + 4 * pa + pr] = f;
+        }
+    };
+
+    // ---- phase B of chunk c (PH = c % 2 fixes the ring slots at compile time): push the chunk's rows through the
+    // register windows.  Pushing row r completes interface (r-4)+1/2 (f+ rows r-7..r-1, f- rows r-6..r) and point r-4.
+    auto phaseB = [&](const int lc, auto ph) {
+        constexpr int PH = decltype(ph)::value;
+        const int r0 = MR * (cbeg + lc);   // first padded row of the chunk
+        // J of the four points this walker completes in this chunk (padded rows r0-4 .. r0-1; the first chunk
+        // completes nothing that is kept)
         double Jw[MR];
         if (KIND != OCFD_GRID_CURVILINEAR) {
             const int i0 = max(r0 - OCFD_NG, 0);
 #pragma unroll
             for (int e = 0; e < MR; ++e) Jw[e] = jrow.at(g, i0, e);
-        }
-        tma::mbar_wait(&bars[s], (c / MNST) & 1);
-        if (KIND == OCFD_GRID_CURVILINEAR) {
-            // the metric box lands densely: field stride = its own row count x MAC
-            const int mi = mfull ? tid : pa, mfs = mfull ? MPTS : MAC;
-            if (validA) {
-                const double *mp = sU + 6 * MPTS + mi;
-                k1 = mp[0]; k2 = mp[mfs]; k3 = mp[2 * mfs]; sig = mp[3 * mfs];
-            }
-            const double *jp = sJ + ((c + MNJ - 1) % MNJ) * MPTS;   // arrived with chunk c-1 (rows r0-4 .. r0-1)
+        } else {
+            const double *jp = sJ + ((lc + MNJ - 1) % MNJ) * MPTS;   // arrived with chunk c-1 (rows r0-4 .. r0-1)
 #pragma unroll
-            for (int e = 0; e < MR; ++e) Jw[e] = DIR == 0 ? jp[wa * MR + e] : jp[(mfull ? e * MAC : 0) + wa];
+            for (int e = 0; e < MR; ++e) Jw[e] = jp[(mfull ? e * MAC : 0) + wa];
         }
-
-        // ---- phase A: split fluxes of the chunk's points; pf(r) = scheme flag of the interface between rows r-1, r
-        if (producer) {
-            double *dst = sF + sfi;
-            if (validA) {
-                double u, v, w, cc;
-                const double rho = sU[tid];
-                prim_from_cons(gs, rho, sU[MPTS + tid], sU[2 * MPTS + tid], sU[3 * MPTS + tid], sU[4 * MPTS + tid], u, v, w, cc);
-                sw_split_store<KIND, DIR>(gs, rho, u, v, w, cc, k1, k2, k3, sig, dst, MPTS);
-            } else {
-#pragma unroll
-                for (int q = 0; q < 10; ++q) dst[q * MPTS] = 0.0;
-            }
-            if (SCHEME == OCFD_HYBRID) {
-                unsigned char f = 0;
-                if (rowA >= OCFD_NG && rowA <= nd + OCFD_NG) {   // interfaces -1/2 .. nd-1/2 (eq. 42, R-12)
-                    const double *thp =
-                        pr > 0 ? sU + 5 * MPTS + tid - (DIR == 0 ? 1 : MAC)
-                               : sIn + ((c + MNST - 1) % MNST) * MSTG + 5 * MPTS + (DIR == 0 ? tid + MR - 1 : (MR - 1) * MAC + pa);
-                    f = (unsigned char)iface_flag(gs, *thp, sU[5 * MPTS + tid]);
-                }
-                sFl[4 * pa + pr] = f;
-            }
-        }
-        __syncthreads();
-        // the stage of chunk c-1 is free now (phase A of this chunk read its last theta row)
-        if (tid == 0 && c + 2 < nch && c > 0) issue(c + 2);
-
-        // ---- phase B: push the chunk's rows through the register windows
-        // pushing row r completes interface (r-4)+1/2 (f+ rows r-7..r-1, f- rows r-6..r) and with it point r-4
         double *so = sO + PH * 5 * MPTS + wm * MPTS + (DIR == 0 ? wa * MR : wa);
-        const double *fpn = sF + wm * MPTS, *fmn = sF + (wm + 5) * MPTS;
+        const double *fpn = sF + PH * 10 * MPTS + wm * MPTS, *fmn = fpn + 5 * MPTS;
         double out[MR];
         bool fast = SCHEME == OCFD_UD7;
         unsigned cur = 0;
         if (SCHEME == OCFD_HYBRID) {
-            const unsigned w = reinterpret_cast<const unsigned *>(sFl)[wa];
+            const unsigned w = reinterpret_cast<const unsigned *>(sFl + PH * 4 * MAC)[wa];
             const unsigned pc = (w & 3u) | ((w >> 6) & 0xcu) | ((w >> 12) & 0x30u) | ((w >> 18) & 0xc0u);
             // the interfaces completed in this chunk: pf(r0-3), pf(r0-2), pf(r0-1), pf(r0)
             cur = ((pprev >> 2) | (pc << 6)) & 0xffu;
@@ -278,22 +281,38 @@ __global__ void __launch_bounds__(MNT, SCHEME == OCFD_HYBRID ? 3 : 4)
             reinterpret_cast<double2 *>(so)[0] = make_double2(out[0], out[1]);
             reinterpret_cast<double2 *>(so)[1] = make_double2(out[2], out[3]);
         }
+    };
+
+    // One CTA barrier per chunk: between two barriers the CTA runs phase A of chunk c+1 and phase B of chunk c (the
+    // split fluxes are double-buffered), so the warp that has no phase-A work and the warps that finish early always
+    // find work of the other kind.  After the barrier: the output tile of chunk c leaves, and the boxes of chunk c+3
+    // are requested into the stage of chunk c (phase A of chunk c+1 has read its last theta row).
+    auto interval = [&](const int lc, auto ph) {
+        constexpr int PH = decltype(ph)::value;
+        if (lc + 1 < nch) phaseA(lc + 1);
+        phaseB(lc, ph);
         tma::fence_proxy_async();
+        // the store of chunk c-1 has finished reading the tile that phase B of chunk c+1 is about to overwrite (it was
+        // issued one interval ago)
+        if (tid == MTMA) tma::store_wait_read<0>();
         __syncthreads();
-        if (tid == 0 && r0 + MR - 1 >= 2 * OCFD_NG) {
-            const int o = r0 - 2 * OCFD_NG;   // interior index of the first completed point (negative rows are clipped)
-            if (DIR == 0) tma::store4(&tm_out, sO + PH * 5 * MPTS, o, a0, cross, 0);
-            else tma::reduce_add4(&tm_out, sO + PH * 5 * MPTS, a0, DIR == 1 ? o : cross, DIR == 2 ? o : cross, 0);
-            tma::store_commit();
-            tma::store_wait_read<1>();   // the other output tile is free for the next chunk
+        if (tid == MTMA) {
+            const int o = MR * (cbeg + lc) - 2 * OCFD_NG;   // interior index of the first point completed by this chunk
+            if (o >= o0) {                                  // (the first two chunks of a segment only fill the windows)
+                if (DIR == 0) tma::store4(&tm_out, sO + PH * 5 * MPTS, o, a0, cross, 0);
+                else tma::reduce_add4(&tm_out, sO + PH * 5 * MPTS, a0, DIR == 1 ? o : cross, DIR == 2 ? o : cross, 0);
+                tma::store_commit();
+            }
+            if (lc + 3 < nch) issue(lc + 3);
         }
     };
-    if (tid == 0 && nch > 2) issue(2);
-    for (int c = 0; c < nch; c += 2) {
-        chunk(c, std::integral_constant<int, 0>());
-        if (c + 1 < nch) chunk(c + 1, std::integral_constant<int, 1>());
+    phaseA(0);
+    __syncthreads();
+    for (int lc = 0; lc < nch; lc += 2) {
+        interval(lc, std::integral_constant<int, 0>());
+        if (lc + 1 < nch) interval(lc + 1, std::integral_constant<int, 1>());
     }
-    if (tid == 0) tma::store_wait_all<0>();
+    if (tid == MTMA) tma::store_wait_all<0>();
 }
 
 template <int KIND, int SCHEME, int DIR>
@@ -302,12 +321,22 @@ ocfd_status launch_march(ocfd_ctx *c) {
     if (!ocfd_smem_optin(c, (const void *)k_inviscid_march<KIND, SCHEME, DIR>, M_SMEM)) return OCFD_ECUDA;
     const int ncross = DIR == 2 ? g.ny : g.nz;
     if (ncross > 65535) return OCFD_EINVAL;
-    dim3 grd(((DIR == 0 ? g.ny : g.nx) + MAC - 1) / MAC, ncross, 1);
+    const int nd = DIR == 0 ? g.nx : DIR == 1 ? g.ny : g.nz, ntile = ((DIR == 0 ? g.ny : g.nx) + MAC - 1) / MAC;
+    // Segments along the march: as few as give every SM's three CTA slots about eight CTAs to work through (a CTA that
+    // marches 2000 rows runs for a millisecond, and the SMs that finish their last one early then idle), never shorter
+    // than 128 rows (each segment re-stages 8 rows); "march_seg" of ocfd_set_tuning overrides (A/B runs).
+    int nseg = 1;
+    while ((long long)ntile * ncross * nseg < 24ll * c->nsm && nd / (nseg + 1) >= 128) ++nseg;
+    if (c->tune.march_seg > 0) nseg = c->tune.march_seg;
+    int seglen = ((nd + nseg - 1) / nseg + MR - 1) / MR * MR;
+    if (seglen < 2 * MR) seglen = 2 * MR;
+    nseg = (nd + seglen - 1) / seglen;
+    dim3 grd(ntile, ncross, nseg);
     OCFD_T0(c, K_INV_X + DIR);
     const MarchMaps &M = c->march;
     const int mfull = DIR != 2 || g.msk != 0;
     k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.U[DIR], M.th[DIR], M.out[DIR],
-                                                                        M.met[DIR], M.metJ[DIR], mfull);
+                                                                        M.met[DIR], M.metJ[DIR], mfull, seglen);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
@@ -342,8 +371,15 @@ bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
                 const long long mdim[4] = {g.nxp, g.nyp, g.msk ? g.nzp : 1, 5};
                 const int mz = d == 2 && g.msk ? MR : 1;
                 const int m4[4] = {bx, by, mz, 4}, m1[4] = {bx, by, mz, 1};
-                if (!ocfd_tma_encode(&M.met[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m4, d == 0)) return false;
-                if (!ocfd_tma_encode(&M.metJ[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m1, d == 0)) return false;
+                if (d == 0) {   // y-contiguous copy [5][planes][nxp][nypT]: boxes of 4 rows of 32 lines
+                    const long long tdim[4] = {g.nyp, g.nxp, g.msk ? g.nzp : 1, 5};
+                    const int t4[4] = {MAC, MR, 1, 4}, t1[4] = {MAC, MR, 1, 1};
+                    if (!ocfd_tma_encode(&M.met[d], g.atabT, tdim, g.nypT, (long long)g.nxp * g.nypT, g.atabT_fs, t4)) return false;
+                    if (!ocfd_tma_encode(&M.metJ[d], g.atabT, tdim, g.nypT, (long long)g.nxp * g.nypT, g.atabT_fs, t1)) return false;
+                } else {
+                    if (!ocfd_tma_encode(&M.met[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m4)) return false;
+                    if (!ocfd_tma_encode(&M.metJ[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m1)) return false;
+                }
             } else {   // unused, but the kernel takes the parameters
                 M.met[d] = M.metJ[d] = CUtensorMap();
             }

@@ -5,7 +5,7 @@
 
 namespace {
 
-__global__ void k_alpha_tables(GridDesc g, double *__restrict__ tab, long long npts) {
+__global__ void k_alpha_tables(GridDesc g, double *__restrict__ tab, double *__restrict__ tabT, long long npts) {
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long id = (long long)blockIdx.x * blockDim.x + threadIdx.x; id < npts; id += stride) {
         const double J = g.met[9][id];
@@ -19,6 +19,16 @@ __global__ void k_alpha_tables(GridDesc g, double *__restrict__ tab, long long n
             t[2 * g.atab_fs] = a3 / sigma;
             t[3 * g.atab_fs] = sigma;
             t[4 * g.atab_fs] = J;
+            if (d == 0) {   // the copy of direction 0 with y contiguous (x sweep)
+                const int ip = (int)(id % g.nxp), jp = (int)((id / g.nxp) % g.nyp);
+                const long long pl = id / g.sz;
+                double *tt = tabT + (pl * g.nxp + ip) * g.nypT + jp;
+                tt[0] = a1 / sigma;
+                tt[g.atabT_fs] = a2 / sigma;
+                tt[2 * g.atabT_fs] = a3 / sigma;
+                tt[3 * g.atabT_fs] = sigma;
+                tt[4 * g.atabT_fs] = J;
+            }
         }
     }
 }
@@ -36,7 +46,7 @@ ocfd_status launch_metric_tables(ocfd_ctx *c) {
         const long long npts = g.atab_fs;
         int blocks = (int)((npts + 255) / 256);
         if (blocks > c->nsm * 16) blocks = c->nsm * 16;
-        k_alpha_tables<<<blocks, 256, 0, c->stream>>>(g, c->mtab, npts);
+        k_alpha_tables<<<blocks, 256, 0, c->stream>>>(g, c->mtab, const_cast<double *>(g.atabT), npts);
         if (cudaGetLastError() != cudaSuccess) return OCFD_ECUDA;
     } else if (g.kind == OCFD_GRID_STRETCHED) {
         const int n[3] = {g.nxp, g.nyp, g.nzp};

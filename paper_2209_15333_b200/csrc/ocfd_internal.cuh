@@ -31,6 +31,12 @@ struct GridDesc {
     //   uniform:     ua[d] = dx dy dz / spacing of axis d  (= d_d/J)
     const double *atab[3];
     long long atab_fs;     // field stride of atab (doubles)
+    // curvilinear: the table of direction 0 once more with y contiguous, [5][planes][nxp][nypT] (nypT = nyp rounded up
+    // to even): the x sweep stages 32 lines x 4 x-points per chunk, which are 4 rows of 256 bytes in this copy instead
+    // of 32 rows of 32 bytes (the TMA engine works row by row)
+    const double *atabT;
+    long long atabT_fs;
+    int nypT;
     const double *rmet[3];
     double ua[3];
 };
@@ -85,6 +91,7 @@ struct Tuning {
     int zchunk_f;    // planes per CTA of viscous pass 1 (0 automatic)
     int zchunk_d;    // ... of viscous pass 2
     int zchunk_s;    // ... of the shock sensor
+    int march_seg;   // segments per pencil of the marching sweeps (0 automatic)
 };
 
 struct ocfd_ctx {
