@@ -191,28 +191,33 @@ static ocfd_status flux_and_sensor(ocfd_ctx *c, const double *U) {
 
 // rows a2-a7; rk_stage >= 0 additionally folds the RK3 stage update (a8) into the last kernel that touches dU.
 // Order: viscous pass 1 (+ sensor) first -- it depends on U only --, then the sweeps, then viscous pass 2 (+ RK3).
-static ocfd_status rhs_impl(ocfd_ctx *c, double *U, double *dU, int rk_stage, double dt) {
+static ocfd_status rhs_impl(ocfd_ctx *c, const double *U, double *dU, int rk_stage, double dt, const RkBufs &rk) {
     ocfd_status st;
     if ((st = flux_and_sensor(c, U)) != OCFD_OK) return st;
     if ((st = launch_inviscid(c, U, dU)) != OCFD_OK) return st;
-    if (!c->p.inviscid) return launch_viscous_div(c, dU, U, dt, rk_stage);
-    if (rk_stage >= 0) return launch_rk_update(c, c->Un, U, dU, dt, rk_stage);
+    if (!c->p.inviscid) return launch_viscous_div(c, dU, rk, dt, rk_stage);
+    if (rk_stage >= 0) return launch_rk_update(c, rk.Un, rk.Uin, rk.out, dU, dt, rk_stage);
     return OCFD_OK;
 }
 
 ocfd_status ocfd_rhs(ocfd_ctx *c, const double *U, double *dU) {
     if (!live(c)) return OCFD_ESTATE;
     if (!U || !dU || U == dU) return OCFD_EINVAL;
-    return rhs_impl(c, const_cast<double *>(U), dU, -1, 0.0);  // rk_stage < 0: U is only read
+    return rhs_impl(c, U, dU, -1, 0.0, RkBufs{nullptr, nullptr, nullptr});  // rk_stage < 0: no update
 }
 
 ocfd_status ocfd_rk3_step(ocfd_ctx *c, double *U, double dt) {
     if (!live(c)) return OCFD_ESTATE;
     if (!U || !(dt == dt)) return OCFD_EINVAL;
     ocfd_status st;
+    // eq. 45 without a copy of the state: U keeps U^n through the step, the intermediate states live in the second
+    // buffer B, and the last stage writes U^(n+1) over U^n (point-wise, so in place is safe)
+    double *B = c->Un;
+    const RkBufs rk[3] = {{nullptr, U, B}, {U, B, B}, {U, B, U}};
     for (int s = 0; s < 3; ++s) {
-        if ((st = launch_fill_ghosts(c, U)) != OCFD_OK) return st;
-        if ((st = rhs_impl(c, U, c->dUw, s, dt)) != OCFD_OK) return st;
+        double *cur = s == 0 ? U : B;
+        if ((st = launch_fill_ghosts(c, cur)) != OCFD_OK) return st;
+        if ((st = rhs_impl(c, cur, c->dUw, s, dt, rk[s])) != OCFD_OK) return st;
     }
     return launch_fill_ghosts(c, U);
 }

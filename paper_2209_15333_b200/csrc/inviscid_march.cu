@@ -1,19 +1,21 @@
 // Rows a2 + a4 + a5 of ONE sweep direction: primitives from U, Steger-Warming split (eq. 19-29),
 // UD7 / WENO7 / WENO5 reconstruction (eq. 41) and the conservative flux difference, as a MARCHING
-// kernel.  It is the z sweep of every run (the x and y sweeps are fused in inviscid_xy.cu); its x and y instances
-// remain selectable (ocfd_set_tuning "xy_fused" = 0) as the unfused reference for A/B measurements.
+// kernel.  It runs the x, y and z sweeps of every run in component-wise variables (ocfd_set_tuning "xy_fused" = 1
+// replaces the x and y launches by the fused kernel of inviscid_xy.cu, an experiment that measured slower).
 //
-// A CTA owns MAC = 32 pencils (32 consecutive x) of one cross index and walks along the sweep direction through all
-// nd + 8 padded rows in chunks of MR = 4 rows.  Every chunk:
-//   TMA      the state of the chunk (the five conserved fields as ONE box; theta if hybrid) arrives in a ring of
-//            MNST = 3 stages that runs two chunks ahead of the arithmetic (one mbarrier per stage);
+// A CTA owns MAC = 32 pencils (32 consecutive x; for the x sweep 32 consecutive y lines) of one cross index and walks
+// along the sweep direction through the padded rows of its segment in chunks of MR = 4 rows.  Per chunk c:
+//   TMA      the state of the chunk (the five conserved fields as ONE box; theta if hybrid; on curvilinear grids the
+//            metric tables k, sigma and J) arrives in a ring of MNST = 3 stages, requested three chunks ahead by one
+//            thread of the warp that has no phase-A work (one mbarrier per stage);
 //   phase A  one thread per point of the chunk: u, v, w, c from the conserved variables, then the split fluxes
-//            f+-[5] -> shared memory.  Each point is split exactly once per sweep (no halo recomputation) and neither
-//            the primitives nor f+- ever reach HBM (the paper materialises f+-, L549);
+//            f+-[5] -> shared memory (double-buffered).  Each point is split exactly once per sweep (no halo
+//            recomputation) and neither the primitives nor f+- ever reach HBM (the paper materialises f+-, L549);
 //   phase B  one thread per (pencil, component): the 7-point windows of f+ and f- live in registers for the whole
 //            march, each new row costs two shared-memory loads; h_{i+1/2} is formed as soon as row i+4 has been
 //            pushed and -J (h_{i+1/2} - h_{i-1/2}) goes to an output tile in shared memory;
-//   TMA      the output tile leaves by one reduce-add per chunk (dU += at the L2; the x sweep has written dU before).
+//   TMA      the output tile leaves by one tensor store (x sweep: it writes dU) or one reduce-add (y, z: dU += at the L2).
+// Between two CTA barriers the CTA runs phase A of chunk c+1 and phase B of chunk c: ONE barrier per chunk.
 // The output tensor map covers the interior of dU only, so the rows before the first interior point, ragged tiles and
 // ghosts are clipped by the hardware.
 #include "ocfd_internal.cuh"

@@ -107,7 +107,7 @@ struct ocfd_ctx {
     // workspace carve-up (device pointers)
     double *theta;   // [np]
     double *Fv;      // [12][np]
-    double *Un;      // [5][np]
+    double *Un;      // [5][np]: the second state buffer of ocfd_rk3_step (holds U^(1), U^(2); the user's U keeps U^n)
     double *dUw;     // [5][np]
     double *scal;    // small scalar area (wavespeed result)
     double *mtab;    // derived metric tables (see GridDesc)
@@ -218,8 +218,12 @@ ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU);
 ocfd_status launch_inviscid_xy(ocfd_ctx *c, const double *U, double *dU);
 ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int dir);
 ocfd_status launch_viscous_flux(ocfd_ctx *c, const double *U, bool sensor);
-ocfd_status launch_viscous_div(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage);
-ocfd_status launch_rk_update(ocfd_ctx *c, double *Un, double *U, const double *dU, double dt, int stage);
+// RK3 buffers of one stage (eq. 45): out <- a_s Un + b_s (Uin + dt dU); ocfd_rk3_step rotates them so that no stage
+// copies the state (stage 0: user's U -> second buffer; stage 1: in place in the second buffer; stage 2: -> user's U)
+struct RkBufs { const double *Un, *Uin; double *out; };
+ocfd_status launch_viscous_div(ocfd_ctx *c, double *dU, const RkBufs &rk, double dt, int rk_stage);
+ocfd_status launch_rk_update(ocfd_ctx *c, const double *Un, const double *Uin, double *out, const double *dU, double dt,
+                             int stage);
 ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
 
 // Raise the dynamic shared-memory limit of `kernel` to `bytes` once per context (the attribute lives in the device

@@ -28,13 +28,17 @@ struct VG {                                    // geometry of the scheme of orde
     static constexpr int W = 2 * H + 1;        // z window
 };
 
+// central-difference coefficients in constant memory: every DFMA takes its coefficient as a constant-bank operand (an
+// immediate fp64 constant costs two moves per use)
+__constant__ double c_d6[3] = {45.0 / 60.0, -9.0 / 60.0, 1.0 / 60.0};                               // 6th order (L313)
+__constant__ double c_d8[4] = {672.0 / 840.0, -168.0 / 840.0, 32.0 / 840.0, -3.0 / 840.0};         // 8th order: 4/5, -1/5, 4/105, -1/280
+
 __device__ __forceinline__ double d1c(double m3, double m2, double m1, double p1, double p2, double p3) {
-    return (45.0 * (p1 - m1) - 9.0 * (p2 - m2) + (p3 - m3)) * (1.0 / 60.0);
+    return fma(c_d6[2], p3 - m3, fma(c_d6[1], p2 - m2, c_d6[0] * (p1 - m1)));
 }
-// 8th-order central: 4/5, -1/5, 4/105, -1/280
 __device__ __forceinline__ double d1c8(double m4, double m3, double m2, double m1, double p1, double p2, double p3,
                                        double p4) {
-    return (672.0 * (p1 - m1) - 168.0 * (p2 - m2) + 32.0 * (p3 - m3) - 3.0 * (p4 - m4)) * (1.0 / 840.0);
+    return fma(c_d8[3], p4 - m4, fma(c_d8[2], p3 - m3, fma(c_d8[1], p2 - m2, c_d8[0] * (p1 - m1))));
 }
 // interior stencil of order ORDER on a line (p points at the position, stride st)
 template <int ORDER>
@@ -87,11 +91,23 @@ struct VF {
     static_assert((STAGE * 8) % 128 == 0, "TMA destinations must stay 128-byte aligned");
 };
 
-// (rho, rho u, rho v, rho w, E) -> (T, u, v, w, p) of the points of one staged plane, in place
+// (rho, rho u, rho v, rho w, E) -> (T, u, v, w, p) of one staged plane, in place.  Only the points a stencil reaches are
+// converted: the own rows with their x halo and the y-halo rows above the own columns (496 of the 560 staged points
+// for the 6th-order scheme: two rounds of the 256 threads instead of three); the corners stay raw and are never read.
 template <int ORDER>
 __device__ __forceinline__ void convert_plane(const GasDesc &gs, double *st, int tid) {
-    constexpr int FLD = VF<ORDER>::FLD;
-    for (int p = tid; p < FLD; p += VNT) {
+    constexpr int FLD = VF<ORDER>::FLD, H = VG<ORDER>::H, WX = TX + 2 * H, N1 = TY * WX, N = N1 + 2 * H * TX;
+    for (int q = tid; q < N; q += VNT) {
+        int row, col;
+        if (q < N1) {
+            row = H + q / WX;
+            col = 4 - H + q % WX;
+        } else {
+            const int hr = (q - N1) / TX;
+            row = hr < H ? hr : hr + TY;
+            col = 4 + (q - N1) % TX;
+        }
+        const int p = row * BXW + col;
         const double rho = st[p];
         const double ir = fast_rcp_pos(rho);
         const double u = st[FLD + p] * ir, v = st[2 * FLD + p] * ir, w = st[3 * FLD + p] * ir;
@@ -135,7 +151,10 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     const int ipc = min(i, g.nx - 1) + OCFD_NG, jpc = min(j, g.ny - 1) + OCFD_NG;
     const long long col = (long long)jpc * g.sy + ipc;
     const int ctr = (ty + H) * BXW + tx + 4;  // own point inside a staged field
-    double w[4][2 * H + 1];
+    // Only the H planes BELOW the current one live in registers (wlo[a][q] = plane k-H+q); the current plane and the H
+    // planes above it are read from the ring, where they sit converted anyway: 12 registers of window per field set
+    // instead of 28, and 3 values to shift per field and plane instead of 6.
+    double wlo[4][H];
     double pm = 0.0;                           // p of plane k-1 (sensor)
 #pragma unroll
     for (int q = 0; q < H; ++q) {
@@ -143,7 +162,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
         const double rho = __ldg(U + id), ir = fast_rcp_pos(rho);
         const double u = __ldg(U + g.np + id) * ir, v = __ldg(U + 2 * g.np + id) * ir, ww = __ldg(U + 3 * g.np + id) * ir;
         const double pr = gs.gm1 * (__ldg(U + 4 * g.np + id) - 0.5 * rho * (u * u + v * v + ww * ww));
-        w[0][q + 1] = gs.gM2 * pr * ir; w[1][q + 1] = u; w[2][q + 1] = v; w[3][q + 1] = ww;
+        wlo[0][q] = gs.gM2 * pr * ir; wlo[1][q] = u; wlo[2][q] = v; wlo[3][q] = ww;
         pm = pr;
     }
     __syncthreads();  // barriers initialised
@@ -155,11 +174,6 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
         convert_plane<ORDER>(gs, ring + q * VF_STAGE, tid);
     }
     __syncthreads();
-#pragma unroll
-    for (int q = 0; q < H; ++q) {
-#pragma unroll
-        for (int a = 0; a < 4; ++a) w[a][q + H + 1] = ring[q * VF_STAGE + a * FLD + ctr];
-    }
     // whole-tile tests: away from aperiodic faces every point takes the central stencil and no row test is needed
     const bool xin = g.periodic[0] || (i0 >= H && i0 + TX <= g.nx - H);
     const bool yin = g.periodic[1] || (j0 >= H && j0 + TY <= g.ny - H);
@@ -171,23 +185,33 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
         for (int d = 0; d < 3; ++d) Met<KIND>::row(g, d, i + OCFD_NG, j + OCFD_NG, 0, m[d][0], m[d][1], m[d][2]);
         iJ = 1.0 / Met<KIND>::J(g, i + OCFD_NG, j + OCFD_NG, 0);
     }
-    for (int k = k0; k < k1; ++k) {
+    const int ip = i + OCFD_NG, jp = j + OCFD_NG;
+    long long id = (long long)(k0 + OCFD_NG) * g.sz + (long long)jp * g.sy + ip;   // this thread's point of plane k
+    int sk = 0;                                                                    // ring stage of plane k
+    for (int k = k0; k < k1; ++k, id += g.sz, sk = sk + 1 == VF_NST ? 0 : sk + 1) {
         const int kp = k + OCFD_NG;
-        const int sn = (k + H - k0) % VF_NST;      // plane k+H: converted during the previous iteration (or above)
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-#pragma unroll
-            for (int q = 0; q < 2 * H; ++q) w[a][q] = w[a][q + 1];
-            w[a][2 * H] = ring[sn * VF_STAGE + a * FLD + ctr];
-        }
         if (own) {
-            const double *sp = ring + ((k - k0) % VF_NST) * VF_STAGE + ctr;
-            const int ip = i + OCFD_NG, jp = j + OCFD_NG;
-            const long long id = (long long)kp * g.sz + (long long)jp * g.sy + ip;
+            const double *sp = ring + sk * VF_STAGE + ctr;
+            // z window of the four fields: planes k-H .. k-1 from registers, k .. k+H from the ring (plane k+H was
+            // converted during the previous iteration, or before the loop)
+            double w[4][2 * H + 1];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+#pragma unroll
+                for (int q = 0; q < H; ++q) w[a][q] = wlo[a][q];
+#pragma unroll
+                for (int q = 0; q <= H; ++q) {
+                    const int sq = sk + q < VF_NST ? sk + q : sk + q - VF_NST;
+                    w[a][H + q] = ring[sq * VF_STAGE + a * FLD + ctr];
+                }
+#pragma unroll
+                for (int q = 0; q + 1 < H; ++q) wlo[a][q] = wlo[a][q + 1];
+                wlo[a][H - 1] = w[a][H];
+            }
             if (SENSOR) {
                 // theta = phi_i + phi_j + phi_k, phi = |p- - 2 p0 + p+| / (p- + 2 p0 + p+); one division for the three
                 const double *cp = sp + 4 * FLD;
-                const double p0 = cp[0], pp = ring[((k + 1 - k0) % VF_NST) * VF_STAGE + 4 * FLD + ctr];
+                const double p0 = cp[0], pp = ring[(sk + 1 < VF_NST ? sk + 1 : 0) * VF_STAGE + 4 * FLD + ctr];
                 const double t0 = p0 + p0;
                 const double ni = fabs(t0 - cp[-1] - cp[1]), di = t0 + cp[-1] + cp[1];
                 const double nj = fabs(t0 - cp[-BXW] - cp[BXW]), dj = t0 + cp[-BXW] + cp[BXW];
@@ -287,8 +311,7 @@ __global__ void __launch_bounds__(VNT, 1)
     k_viscous_div(const GridDesc g, const __grid_constant__ CUtensorMap tm_F, const __grid_constant__ CUtensorMap tm_G,
                   const __grid_constant__ CUtensorMap tm_H, const __grid_constant__ CUtensorMap tm_dU,
                   const __grid_constant__ CUtensorMap tm_U, const __grid_constant__ CUtensorMap tm_Un,
-                  const double *__restrict__ Fv, double *__restrict__ dU, double *__restrict__ U,
-                  double *__restrict__ Un, double dt, int zchunk) {
+                  const double *__restrict__ Fv, double *__restrict__ dU, double *Uout, double dt, int zchunk) {
     constexpr int HH = VG<ORDER>::H, BYH = VG<ORDER>::BYH, VD_G = VD<ORDER>::G, VD_STAGE = VD<ORDER>::STAGE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
@@ -362,13 +385,14 @@ __global__ void __launch_bounds__(VNT, 1)
                 for (int m = 0; m < 5; ++m) {
                     const long long q = m * g.np + id;
                     const double u = sU[m * TY * TX + ctr];
+                    // (Uout may be the buffer tm_U or tm_Un reads: the boxes of this plane have landed, and no other
+                    // CTA reads these points)
                     if (RK == 1) {
-                        __stcs(Un + q, u);
-                        __stcs(U + q, u + dt * acc[m]);
+                        __stcs(Uout + q, u + dt * acc[m]);
                     } else if (RK == 2) {
-                        __stcs(U + q, 0.75 * sUn[m * TY * TX + ctr] + 0.25 * (u + dt * acc[m]));
+                        __stcs(Uout + q, 0.75 * sUn[m * TY * TX + ctr] + 0.25 * (u + dt * acc[m]));
                     } else {
-                        __stcs(U + q, (1.0 / 3.0) * sUn[m * TY * TX + ctr] + (2.0 / 3.0) * (u + dt * acc[m]));
+                        __stcs(Uout + q, (1.0 / 3.0) * sUn[m * TY * TX + ctr] + (2.0 / 3.0) * (u + dt * acc[m]));
                     }
                 }
             }
@@ -406,6 +430,7 @@ bool encode_flux_map(ocfd_ctx *c, const double *U) {
     return true;
 }
 
+// M.Un describes the context's second state buffer, M.U the caller's U (re-encoded when the pointer changes)
 bool encode_div_maps(ocfd_ctx *c, const double *dU, const double *U) {
     const GridDesc &g = c->g;
     ViscMaps &M = c->visc;
@@ -432,27 +457,30 @@ bool encode_div_maps(ocfd_ctx *c, const double *dU, const double *U) {
 }
 
 template <int KIND, int RK, int ORDER>
-ocfd_status launch_div(ocfd_ctx *c, dim3 grd, dim3 blk, double *dU, double *U, double dt, int zc) {
+ocfd_status launch_div(ocfd_ctx *c, dim3 grd, dim3 blk, double *dU, const RkBufs &rk, double dt, int zc) {
     if (!ocfd_smem_optin(c, (const void *)k_viscous_div<KIND, RK, ORDER>, VD<ORDER>::SMEM)) return OCFD_ECUDA;
     const ViscMaps &M = c->visc;
-    k_viscous_div<KIND, RK, ORDER><<<grd, blk, VD<ORDER>::SMEM, c->stream>>>(c->g, M.F, M.G, M.H, M.dU, RK ? M.U : M.dU, M.Un, c->Fv, dU, U,
-                                                             c->Un, dt, zc);
+    auto map_of = [&](const double *p) -> const CUtensorMap & { return p == c->Un ? M.Un : M.U; };
+    k_viscous_div<KIND, RK, ORDER><<<grd, blk, VD<ORDER>::SMEM, c->stream>>>(
+        c->g, M.F, M.G, M.H, M.dU, RK ? map_of(rk.Uin) : M.dU, RK >= 2 ? map_of(rk.Un) : M.dU, c->Fv, dU, rk.out, dt, zc);
     return OCFD_OK;
 }
 
 template <int KIND, int ORDER>
-ocfd_status launch_div_kind(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
+ocfd_status launch_div_kind(ocfd_ctx *c, double *dU, const RkBufs &rk, double dt, int rk_stage) {
     const GridDesc &g = c->g;
-    if (!encode_div_maps(c, dU, rk_stage >= 0 ? U : nullptr)) return OCFD_ECUDA;
+    // the caller's U is whichever of the stage's buffers is not the context's own
+    const double *user = rk_stage < 0 ? nullptr : rk.Uin != c->Un ? rk.Uin : rk.Un;
+    if (!encode_div_maps(c, dU, user)) return OCFD_ECUDA;
     const int zcd = pick_zchunk(c, 2);
     dim3 blk(TX, TY, 1), grdd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zcd - 1) / zcd);
     OCFD_T0(c, K_VISC_DIV);
     ocfd_status st;
     switch (rk_stage) {
-        case 0: st = launch_div<KIND, 1, ORDER>(c, grdd, blk, dU, U, dt, zcd); break;
-        case 1: st = launch_div<KIND, 2, ORDER>(c, grdd, blk, dU, U, dt, zcd); break;
-        case 2: st = launch_div<KIND, 3, ORDER>(c, grdd, blk, dU, U, dt, zcd); break;
-        default: st = launch_div<KIND, 0, ORDER>(c, grdd, blk, dU, nullptr, 0.0, zcd);
+        case 0: st = launch_div<KIND, 1, ORDER>(c, grdd, blk, dU, rk, dt, zcd); break;
+        case 1: st = launch_div<KIND, 2, ORDER>(c, grdd, blk, dU, rk, dt, zcd); break;
+        case 2: st = launch_div<KIND, 3, ORDER>(c, grdd, blk, dU, rk, dt, zcd); break;
+        default: st = launch_div<KIND, 0, ORDER>(c, grdd, blk, dU, rk, 0.0, zcd);
     }
     if (st != OCFD_OK) return st;
     OCFD_CHECK_LAUNCH(c);
@@ -495,19 +523,19 @@ ocfd_status launch_viscous_flux(ocfd_ctx *c, const double *U, bool sensor) {
     }
 }
 
-// Pass 2 (a7): rk_stage < 0: dU += viscous terms.  rk_stage = 0,1,2: the same, then U <- RK3 stage update (a8) in the
-// same kernel.
-ocfd_status launch_viscous_div(ocfd_ctx *c, double *dU, double *U, double dt, int rk_stage) {
+// Pass 2 (a7): rk_stage < 0: dU += viscous terms.  rk_stage = 0,1,2: the same, then rk.out <- RK3 stage update (a8) in
+// the same kernel.
+ocfd_status launch_viscous_div(ocfd_ctx *c, double *dU, const RkBufs &rk, double dt, int rk_stage) {
     if (c->visc_order == 8) {
         switch (c->g.kind) {
-            case OCFD_GRID_UNIFORM: return launch_div_kind<OCFD_GRID_UNIFORM, 8>(c, dU, U, dt, rk_stage);
-            case OCFD_GRID_STRETCHED: return launch_div_kind<OCFD_GRID_STRETCHED, 8>(c, dU, U, dt, rk_stage);
-            default: return launch_div_kind<OCFD_GRID_CURVILINEAR, 8>(c, dU, U, dt, rk_stage);
+            case OCFD_GRID_UNIFORM: return launch_div_kind<OCFD_GRID_UNIFORM, 8>(c, dU, rk, dt, rk_stage);
+            case OCFD_GRID_STRETCHED: return launch_div_kind<OCFD_GRID_STRETCHED, 8>(c, dU, rk, dt, rk_stage);
+            default: return launch_div_kind<OCFD_GRID_CURVILINEAR, 8>(c, dU, rk, dt, rk_stage);
         }
     }
     switch (c->g.kind) {
-        case OCFD_GRID_UNIFORM: return launch_div_kind<OCFD_GRID_UNIFORM, 6>(c, dU, U, dt, rk_stage);
-        case OCFD_GRID_STRETCHED: return launch_div_kind<OCFD_GRID_STRETCHED, 6>(c, dU, U, dt, rk_stage);
-        default: return launch_div_kind<OCFD_GRID_CURVILINEAR, 6>(c, dU, U, dt, rk_stage);
+        case OCFD_GRID_UNIFORM: return launch_div_kind<OCFD_GRID_UNIFORM, 6>(c, dU, rk, dt, rk_stage);
+        case OCFD_GRID_STRETCHED: return launch_div_kind<OCFD_GRID_STRETCHED, 6>(c, dU, rk, dt, rk_stage);
+        default: return launch_div_kind<OCFD_GRID_CURVILINEAR, 6>(c, dU, rk, dt, rk_stage);
     }
 }
