@@ -144,7 +144,8 @@ ocfd_status ocfd_debug_sensor(ocfd_ctx *ctx, const double *U, double *theta, uns
  * "xy_fused" (0, default: one marching launch per sweep direction; 1: the x and y sweeps run as one kernel, an
  * experiment that is slower on every measured workload), "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a CTA of
  * the viscous passes / the stand-alone sensor marches; 0 automatic, else >= 8), "march_seg" (segments a pencil of the
- * marching sweeps is cut into; 0 automatic).  Unknown key or negative value: OCFD_EINVAL. */
+ * marching sweeps is cut into; 0 automatic), "tile_group" (tiles per column group in the CTA numbering of the viscous
+ * passes; 0 = 16, a value >= the tiles per row gives the plain x-fastest order).  Unknown key or negative value: OCFD_EINVAL. */
 ocfd_status ocfd_set_tuning(ocfd_ctx *ctx, const char *key, int value);
 
 /* sizeof(ocfd_params) as compiled, so that a foreign-language mirror of the struct can check itself. */

@@ -296,6 +296,7 @@ ocfd_status ocfd_set_tuning(ocfd_ctx *c, const char *key, int value) {
     else if (!strcmp(key, "zchunk_div")) c->tune.zchunk_d = value;
     else if (!strcmp(key, "zchunk_sensor")) c->tune.zchunk_s = value;
     else if (!strcmp(key, "march_seg")) c->tune.march_seg = value;
+    else if (!strcmp(key, "tile_group")) c->tune.tile_group = value;
     else return OCFD_EINVAL;
     return OCFD_OK;
 }

@@ -113,8 +113,10 @@ __global__ void __launch_bounds__(MNT, 3)
         if (KIND == OCFD_GRID_CURVILINEAR) {
             const int m2 = DIR == 2 ? (mfull ? MR * c : 0) : (g.msk ? OCFD_NG + cross : 0);
             // (x sweep: the copy of the table with y contiguous, so the box is [4 x][32 lines])
-            tma::load4(dst + 6 * MPTS, &tm_met, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 0);
-            tma::load4(sJ + (lc % MNJ) * MPTS, &tm_metJ, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 4);
+            // z-extruded tables are a few planes that every cross index reads again: ask the L2 to keep them
+            const uint64_t keep = tma::policy_evict_last();
+            tma::load4_hint(dst + 6 * MPTS, &tm_met, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 0, keep);
+            tma::load4_hint(sJ + (lc % MNJ) * MPTS, &tm_metJ, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 4, keep);
         }
         tma::load4(dst, &tm_U, &bars[s], c0, c1, c2, 0);
         if (SCHEME == OCFD_HYBRID) tma::load4(dst + 5 * MPTS, &tm_th, &bars[s], c0, c1, c2, 0);

@@ -92,6 +92,7 @@ struct Tuning {
     int zchunk_d;    // ... of viscous pass 2
     int zchunk_s;    // ... of the shock sensor
     int march_seg;   // segments per pencil of the marching sweeps (0 automatic)
+    int tile_group;  // tiles per column group in the CTA numbering of the viscous passes (0: 16; >= tiles per row: x-fastest)
 };
 
 struct ocfd_ctx {

@@ -20,6 +20,25 @@
 namespace {
 
 constexpr int TX = 32, TY = 8, VNT = TX * TY;  // own points of a tile = threads
+
+// Tile of a CTA.  The hardware hands out CTAs in the order of their linear index; with the plain x-fastest numbering
+// the CTAs resident at one time form two or three full rows of tiles, and most y halos are fetched from HBM twice.
+// Numbering the tiles column group by column group (gw tiles wide, y fastest between the rows of a group) makes the
+// resident set a compact block whose inner halos are found in the L2; rows of a group stay contiguous in memory.
+__device__ __forceinline__ void tile_of_block(int gw, int &bx, int &by) {
+    const int nxt = gridDim.x, nyt = gridDim.y;
+    const int L = blockIdx.x + nxt * blockIdx.y;
+    const int nfull = nxt / gw, rem = nxt - nfull * gw;
+    if (L < nfull * gw * nyt) {
+        const int grp = L / (gw * nyt), r = L - grp * gw * nyt;
+        by = r / gw;
+        bx = grp * gw + (r - by * gw);
+    } else {
+        const int r = L - nfull * gw * nyt;
+        by = r / rem;
+        bx = nfull * gw + (r - by * rem);
+    }
+}
 constexpr int BXW = TX + 8;                    // x extent of a box with x halos (i0-4 .. i0+TX+3)
 template <int ORDER>
 struct VG {                                    // geometry of the scheme of order ORDER (6 or 8)
@@ -123,13 +142,16 @@ __device__ __forceinline__ void convert_plane(const GasDesc &gs, double *st, int
 template <int KIND, int ORDER, bool SENSOR>
 __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     k_viscous_flux(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_U,
-                   const double *__restrict__ U, double *__restrict__ Fv, double *__restrict__ theta, int zchunk) {
+                   const double *__restrict__ U, double *__restrict__ Fv, double *__restrict__ theta, int zchunk,
+                   int tgroup) {
     constexpr int H = VG<ORDER>::H, VF_NST = VF<ORDER>::NST, VF_STAGE = VF<ORDER>::STAGE, FLD = VF<ORDER>::FLD;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + VF_NST * VF_STAGE);
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
-    const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+    int tbx, tby;
+    tile_of_block(tgroup, tbx, tby);
+    const int i0 = tbx * TX, j0 = tby * TY;
     const int i = i0 + tx, j = j0 + ty;
     const bool own = i < g.nx && j < g.ny;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
@@ -311,13 +333,16 @@ __global__ void __launch_bounds__(VNT, 1)
     k_viscous_div(const GridDesc g, const __grid_constant__ CUtensorMap tm_F, const __grid_constant__ CUtensorMap tm_G,
                   const __grid_constant__ CUtensorMap tm_H, const __grid_constant__ CUtensorMap tm_dU,
                   const __grid_constant__ CUtensorMap tm_U, const __grid_constant__ CUtensorMap tm_Un,
-                  const double *__restrict__ Fv, double *__restrict__ dU, double *Uout, double dt, int zchunk) {
+                  const double *__restrict__ Fv, double *__restrict__ dU, double *Uout, double dt, int zchunk,
+                  int tgroup) {
     constexpr int HH = VG<ORDER>::H, BYH = VG<ORDER>::BYH, VD_G = VD<ORDER>::G, VD_STAGE = VD<ORDER>::STAGE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
     uint64_t *bars = reinterpret_cast<uint64_t *>(ring + VD_NST * VD_STAGE);
     const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
-    const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+    int tbx, tby;
+    tile_of_block(tgroup, tbx, tby);
+    const int i0 = tbx * TX, j0 = tby * TY;
     const int i = i0 + tx, j = j0 + ty;
     const bool own = i < g.nx && j < g.ny;
     const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
@@ -402,6 +427,13 @@ __global__ void __launch_bounds__(VNT, 1)
     }
 }
 
+// width of the column groups of tile_of_block: 16 tiles (512 points of x), "tile_group" of ocfd_set_tuning overrides
+int tile_group(const ocfd_ctx *c, unsigned nxt) {
+    int gw = c->tune.tile_group > 0 ? c->tune.tile_group : 16;
+    if (gw > (int)nxt) gw = (int)nxt;
+    return gw;
+}
+
 int pick_zchunk(const ocfd_ctx *c, int pass) {
     const GridDesc &g = c->g;
     // enough blocks to fill the SMs a few times over ...
@@ -462,7 +494,8 @@ ocfd_status launch_div(ocfd_ctx *c, dim3 grd, dim3 blk, double *dU, const RkBufs
     const ViscMaps &M = c->visc;
     auto map_of = [&](const double *p) -> const CUtensorMap & { return p == c->Un ? M.Un : M.U; };
     k_viscous_div<KIND, RK, ORDER><<<grd, blk, VD<ORDER>::SMEM, c->stream>>>(
-        c->g, M.F, M.G, M.H, M.dU, RK ? map_of(rk.Uin) : M.dU, RK >= 2 ? map_of(rk.Un) : M.dU, c->Fv, dU, rk.out, dt, zc);
+        c->g, M.F, M.G, M.H, M.dU, RK ? map_of(rk.Uin) : M.dU, RK >= 2 ? map_of(rk.Un) : M.dU, c->Fv, dU, rk.out, dt, zc,
+        tile_group(c, grd.x));
     return OCFD_OK;
 }
 
@@ -495,7 +528,8 @@ ocfd_status launch_flux(ocfd_ctx *c, const double *U) {
     const int zc = pick_zchunk(c, 1);
     dim3 blk(TX, TY, 1), grd((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + zc - 1) / zc);
     OCFD_T0(c, K_VISC_FLUX);
-    k_viscous_flux<KIND, ORDER, SENSOR><<<grd, blk, VF<ORDER>::SMEM, c->stream>>>(g, c->gas, c->visc.Uf, U, c->Fv, c->theta, zc);
+    k_viscous_flux<KIND, ORDER, SENSOR><<<grd, blk, VF<ORDER>::SMEM, c->stream>>>(g, c->gas, c->visc.Uf, U, c->Fv, c->theta, zc,
+                                                                                  tile_group(c, grd.x));
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
