@@ -301,6 +301,9 @@ def run_ours(args):
         barrier()
     ms = e0.elapsed_time(e1)
     launches = s.launch_count() - n0
+    # row a9 once more, after the timed region, so that its kernel shows up in the per-kernel table (a production run
+    # calls it once per step for dt = CFL / Lambda; the timed steps here use one fixed dt, as the parity runs do)
+    s.max_wavespeed(U)
     per_kernel = s.timing_read()
     s.timing(False)
     finite = bool(torch.isfinite(U).all().item())
@@ -334,7 +337,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel, from the library's per-launch CUDA events over the timed region
     hbm_peak, peak_src = peaks()
     alg = algorithmic(case, flag_hist)
-    tot_kernel_ms = sum(v[0] for v in per_kernel.values())
+    tot_kernel_ms = sum(v[0] for k, v in per_kernel.items() if k != "max_wavespeed")
     clk_mhz = clk.summary()["sm_mhz"]
     kern = {}
     for name, (kms, n) in per_kernel.items():
@@ -342,6 +345,8 @@ def run_ours(args):
             continue
         by, fl = alg[name]
         per_launch_ms = kms / n
+        if name == "max_wavespeed":
+            kms = 0.0          # outside the timed region: no share of the step
         gbs = by * case.npoints / (per_launch_ms * 1e-3) / 1e9
         tfl = fl * case.npoints / (per_launch_ms * 1e-3) / 1e12
         kern[name] = {"ms_per_launch": per_launch_ms, "launches_per_step": n / args.steps, "share": kms / tot_kernel_ms,

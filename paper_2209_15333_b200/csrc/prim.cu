@@ -127,32 +127,44 @@ __global__ void k_flags(GridDesc g, GasDesc gs, int scheme, const double *__rest
     }
 }
 
-// a9: Lambda = max sum_d (|d_x u + d_y v + d_z w| + c |grad d|) over interior points (R-17)
+// a9: Lambda = max sum_d (|d_x u + d_y v + d_z w| + c |grad d|) over interior points (R-17).
+// A thread owns one (i, j) column and walks a chunk of z planes: coalesced along x, no index division per point, and on
+// grids whose metrics do not depend on z (uniform; z-extruded curvilinear maps) the nine metric values and the three
+// square roots |grad d| are fetched and formed once per column instead of once per point.
+constexpr int WS_NT = 128;
 template <int KIND>
-__global__ void __launch_bounds__(256) k_wavespeed(GridDesc g, GasDesc gs, const double *__restrict__ U,
-                                                   unsigned long long *__restrict__ out) {
-    long long n = (long long)g.nx * g.ny * g.nz;
-    long long stride = (long long)gridDim.x * blockDim.x;
+__global__ void __launch_bounds__(WS_NT) k_wavespeed(GridDesc g, GasDesc gs, const double *__restrict__ U,
+                                                     unsigned long long *__restrict__ out, int zchunk) {
+    const int i = blockIdx.x * WS_NT + threadIdx.x, j = blockIdx.y;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
     double best = 0.0;
     bool bad = false;
-    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += stride) {
-        int i = (int)(q % g.nx), j = (int)((q / g.nx) % g.ny), k = (int)(q / ((long long)g.nx * g.ny));
-        int ip = i + OCFD_NG, jp = j + OCFD_NG, kp = k + OCFD_NG;
-        long long id = pidx(g, ip, jp, kp);
-        double rho = U[id], ir = 1.0 / rho;
-        double u = U[g.np + id] * ir, v = U[2 * g.np + id] * ir, w = U[3 * g.np + id] * ir;
-        double p = gs.gm1 * (U[4 * g.np + id] - 0.5 * rho * (u * u + v * v + w * w));
-        double c = sqrt(gs.gM2 * p * ir) * gs.invMa;
-        double s = 0.0;
+    if (i < g.nx) {
+        const int ip = i + OCFD_NG, jp = j + OCFD_NG;
+        const bool fixed = KIND == OCFD_GRID_UNIFORM || (KIND == OCFD_GRID_CURVILINEAR && g.msk == 0);
+        double a[3][3], len[3];
+        auto fetch = [&](int kp) {
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            double a1, a2, a3;
-            Met<KIND>::row(g, d, ip, jp, kp, a1, a2, a3);
-            s += fabs(a1 * u + a2 * v + a3 * w) + c * sqrt(a1 * a1 + a2 * a2 + a3 * a3);
+            for (int d = 0; d < 3; ++d) {
+                Met<KIND>::row(g, d, ip, jp, kp, a[d][0], a[d][1], a[d][2]);
+                len[d] = sqrt(a[d][0] * a[d][0] + a[d][1] * a[d][1] + a[d][2] * a[d][2]);
+            }
+        };
+        if (fixed) fetch(OCFD_NG);
+        long long id = pidx(g, ip, jp, k0 + OCFD_NG);
+        for (int k = k0; k < k1; ++k, id += g.sz) {
+            if (!fixed) fetch(k + OCFD_NG);
+            const double rho = U[id], ir = 1.0 / rho;
+            const double u = U[g.np + id] * ir, v = U[2 * g.np + id] * ir, w = U[3 * g.np + id] * ir;
+            const double p = gs.gm1 * (U[4 * g.np + id] - 0.5 * rho * (u * u + v * v + w * w));
+            const double c = sqrt(gs.gM2 * p * ir) * gs.invMa;
+            double s = 0.0;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) s += fabs(a[d][0] * u + a[d][1] * v + a[d][2] * w) + c * len[d];
+            // fmax drops a NaN operand: a blown-up state (NaN rho or p) must not come back as a finite Lambda
+            bad |= !(s == s);
+            best = fmax(best, s);
         }
-        // fmax drops a NaN operand: a blown-up state (NaN rho or p) must not come back as a finite Lambda
-        bad |= !(s == s);
-        best = fmax(best, s);
     }
     // warp-shuffle max, then one atomic per warp on the ordered bit pattern (all values are >= 0; the quiet-NaN
     // pattern orders above +inf, so one bad point makes the result NaN)
@@ -199,14 +211,18 @@ ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out) {
     const GridDesc &g = c->g;
     unsigned long long *out = (unsigned long long *)c->scal;
     if (cudaMemsetAsync(out, 0, sizeof(unsigned long long), c->stream) != cudaSuccess) return OCFD_ECUDA;
-    long long n = (long long)g.nx * g.ny * g.nz;
-    int blocks = (int)((n + 255) / 256);
-    if (blocks > c->nsm * 16) blocks = c->nsm * 16;
+    if (g.ny > 65535) return OCFD_EINVAL;
+    // z chunks: long enough to amortise the per-column metric work, short enough to fill the SMs a few times over
+    int zc = g.nz;
+    const long long cols = (long long)((g.nx + WS_NT - 1) / WS_NT) * g.ny;
+    while (zc > 32 && cols * ((g.nz + zc - 1) / zc) < 8ll * c->nsm) zc = (zc + 1) / 2;
+    if (zc > 64) zc = 64;
+    const dim3 grd((g.nx + WS_NT - 1) / WS_NT, g.ny, (g.nz + zc - 1) / zc);
     OCFD_T0(c, K_WAVE);
     switch (g.kind) {
-        case OCFD_GRID_UNIFORM: k_wavespeed<OCFD_GRID_UNIFORM><<<blocks, 256, 0, c->stream>>>(g, c->gas, U, out); break;
-        case OCFD_GRID_STRETCHED: k_wavespeed<OCFD_GRID_STRETCHED><<<blocks, 256, 0, c->stream>>>(g, c->gas, U, out); break;
-        default: k_wavespeed<OCFD_GRID_CURVILINEAR><<<blocks, 256, 0, c->stream>>>(g, c->gas, U, out);
+        case OCFD_GRID_UNIFORM: k_wavespeed<OCFD_GRID_UNIFORM><<<grd, WS_NT, 0, c->stream>>>(g, c->gas, U, out, zc); break;
+        case OCFD_GRID_STRETCHED: k_wavespeed<OCFD_GRID_STRETCHED><<<grd, WS_NT, 0, c->stream>>>(g, c->gas, U, out, zc); break;
+        default: k_wavespeed<OCFD_GRID_CURVILINEAR><<<grd, WS_NT, 0, c->stream>>>(g, c->gas, U, out, zc);
     }
     OCFD_CHECK_LAUNCH(c);
     if (cudaMemcpyAsync(host_out, out, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return OCFD_ECUDA;
