@@ -20,17 +20,16 @@ typedef CUresult (*ocfd_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_
                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 // the driver's cuTensorMapEncodeTiled, fetched through the runtime (the library does not link libcuda)
+inline ocfd_encode_fn ocfd_tma_lookup() {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+        return (ocfd_encode_fn)p;
+    return nullptr;
+}
 inline ocfd_encode_fn ocfd_tma_encoder() {
-    static ocfd_encode_fn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = (ocfd_encode_fn)p;
-    }
+    static const ocfd_encode_fn fn = ocfd_tma_lookup();   // initialised once, thread-safe (the entry point is per process)
     return fn;
 }
 
