@@ -389,6 +389,34 @@ def test_results_are_bitwise_reproducible(B):
     s.close()
 
 
+@pytest.mark.parametrize("which", ["ramp", "periodic"])
+def test_launch_shape_knobs_change_no_bit(B, which):
+    """ocfd_set_tuning only re-shapes launches: marches cut into segments (every segment re-stages its first 8 rows and
+    recomputes the interface fluxes there from the same values in the same order), short z chunks of the viscous
+    passes, another CTA numbering.  The result must be the same bits, for one RHS and for a whole RK3 step -- which
+    also exercises the segmented march on a grid small enough to compare whole arrays (the automatic rule only cuts
+    marches on grids as large as configs 4 and 5)."""
+    case = W.ramp(nx=72, ny=44, nz=40, nmodes=12) if which == "ramp" else W.shocked_periodic(40)
+    ref = B.Solver(case)
+    U0 = ref.to_device(case.U0.copy())
+    ref.fill_ghosts(U0)
+    dt = 0.3 * case.cfl / ref.max_wavespeed(U0)
+    a = ref.rhs(U0).clone()
+    Ua = U0.clone()
+    ref.rk3_step(Ua, dt)
+    ref.close()
+    for knobs in ({"march_seg": 3}, {"march_seg": 5, "tile_group": 1}, {"zchunk_flux": 8, "zchunk_div": 8, "tile_group": 2}):
+        s = B.Solver(case)
+        for k, v in knobs.items():
+            s.set_tuning(k, v)
+        b = s.rhs(U0).clone()
+        Ub = U0.clone()
+        s.rk3_step(Ub, dt)
+        s.close()
+        assert bool((a == b).all()), knobs
+        assert bool((Ua == Ub).all()), knobs
+
+
 def test_invalid_parameters_are_refused_without_touching_buffers(B):
     """Argument errors come back as status codes (never exceptions from the library), synchronously."""
     case = W.smooth_periodic(8, 8, 8)
