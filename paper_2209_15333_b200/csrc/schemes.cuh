@@ -36,6 +36,18 @@ __device__ __forceinline__ double fast_rcp_pos(double x) {
     return r;
 }
 
+// sqrt(x) for x > 0 in the normal range: hardware seed of 1/sqrt(x), two Newton steps, one correction of the product
+// (within an ulp or two; the library sqrt costs about twice the instructions)
+__device__ __forceinline__ double fast_sqrt_pos(double x) {
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const double hx = 0.5 * x;
+    r = fma(fma(-hx * r, r, 0.5), r, r);
+    r = fma(fma(-hx * r, r, 0.5), r, r);
+    const double s = x * r;
+    return fma(fma(-s, s, x), 0.5 * r, s);
+}
+
 // Row a2 inside its consumers: velocity and speed of sound of one point from the conserved variables (eq. 8 as
 // corrected, DESIGN R-1; eq. 16: c^2 = T / Ma^2 = gamma p / rho).  No primitive field is ever written to HBM: every
 // kernel that needs u, v, w, c (or T, p) forms them from the U box it has staged anyway.

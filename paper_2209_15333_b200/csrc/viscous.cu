@@ -113,20 +113,39 @@ struct VF {
 // (rho, rho u, rho v, rho w, E) -> (T, u, v, w, p) of one staged plane, in place.  Only the points a stencil reaches are
 // converted: the own rows with their x halo and the y-halo rows above the own columns (496 of the 560 staged points
 // for the 6th-order scheme: two rounds of the 256 threads instead of three); the corners stay raw and are never read.
+// The positions a thread converts are the same in every plane: convert_slots works them out once (-1 = none).
 template <int ORDER>
-__device__ __forceinline__ void convert_plane(const GasDesc &gs, double *st, int tid) {
-    constexpr int FLD = VF<ORDER>::FLD, H = VG<ORDER>::H, WX = TX + 2 * H, N1 = TY * WX, N = N1 + 2 * H * TX;
-    for (int q = tid; q < N; q += VNT) {
+struct ConvSlots {
+    static constexpr int H = VG<ORDER>::H, WX = TX + 2 * H, N1 = TY * WX, N = N1 + 2 * H * TX, ROUNDS = (N + VNT - 1) / VNT;
+    int p[ROUNDS];
+};
+template <int ORDER>
+__device__ __forceinline__ ConvSlots<ORDER> convert_slots(int tid) {
+    using C = ConvSlots<ORDER>;
+    C c;
+#pragma unroll
+    for (int r = 0; r < C::ROUNDS; ++r) {
+        const int q = tid + r * VNT;
         int row, col;
-        if (q < N1) {
-            row = H + q / WX;
-            col = 4 - H + q % WX;
+        if (q < C::N1) {
+            row = C::H + q / C::WX;
+            col = 4 - C::H + q % C::WX;
         } else {
-            const int hr = (q - N1) / TX;
-            row = hr < H ? hr : hr + TY;
-            col = 4 + (q - N1) % TX;
+            const int hr = (q - C::N1) / TX;
+            row = hr < C::H ? hr : hr + TY;
+            col = 4 + (q - C::N1) % TX;
         }
-        const int p = row * BXW + col;
+        c.p[r] = q < C::N ? row * BXW + col : -1;
+    }
+    return c;
+}
+template <int ORDER>
+__device__ __forceinline__ void convert_plane(const GasDesc &gs, double *st, const ConvSlots<ORDER> &slots) {
+    constexpr int FLD = VF<ORDER>::FLD;
+#pragma unroll
+    for (int r = 0; r < ConvSlots<ORDER>::ROUNDS; ++r) {
+        const int p = slots.p[r];
+        if (p < 0) continue;
         const double rho = st[p];
         const double ir = fast_rcp_pos(rho);
         const double u = st[FLD + p] * ir, v = st[2 * FLD + p] * ir, w = st[3 * FLD + p] * ir;
@@ -187,13 +206,14 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
         wlo[0][q] = gs.gM2 * pr * ir; wlo[1][q] = u; wlo[2][q] = v; wlo[3][q] = ww;
         pm = pr;
     }
+    const ConvSlots<ORDER> slots = convert_slots<ORDER>(tid);
     __syncthreads();  // barriers initialised
     // planes k0 .. k0+H: convert, then take the own column of the first H into the window
 #pragma unroll 1
     for (int q = 0; q <= H; ++q) {
         if (k0 + q > last) break;
         tma::mbar_wait(&bars[q], 0);
-        convert_plane<ORDER>(gs, ring + q * VF_STAGE, tid);
+        convert_plane<ORDER>(gs, ring + q * VF_STAGE, slots);
     }
     __syncthreads();
     // whole-tile tests: away from aperiodic faces every point takes the central stencil and no row test is needed
@@ -210,8 +230,14 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     const int ip = i + OCFD_NG, jp = j + OCFD_NG;
     long long id = (long long)(k0 + OCFD_NG) * g.sz + (long long)jp * g.sy + ip;   // this thread's point of plane k
     int sk = 0;                                                                    // ring stage of plane k
-    for (int k = k0; k < k1; ++k, id += g.sz, sk = sk + 1 == VF_NST ? 0 : sk + 1) {
+    // periodic images in x and y: fixed per thread
+    const long long imx = !g.periodic[0] ? 0 : i < H ? g.nx : i >= g.nx - H ? -g.nx : 0;
+    const long long imy = !g.periodic[1] ? 0 : j < H ? g.ny * g.sy : j >= g.ny - H ? -(g.ny * g.sy) : 0;
+    double *Fp = Fv + id;
+    const bool xy_edge = i == 0 || j == 0 || i == g.nx - 1 || j == g.ny - 1;   // touches a face in x or y (theta ghosts)
+    for (int k = k0; k < k1; ++k, id += g.sz, Fp += g.sz, sk = sk + 1 == VF_NST ? 0 : sk + 1) {
         const int kp = k + OCFD_NG;
+        const bool zin = g.periodic[2] || (k >= H && k <= g.nz - 1 - H);   // central stencil along z in this plane
         if (own) {
             const double *sp = ring + sk * VF_STAGE + ctr;
             // z window of the four fields: planes k-H .. k-1 from registers, k .. k+H from the ring (plane k+H was
@@ -242,7 +268,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
                 const double th = fast_div_pos(ni * (dj * dk) + nj * (di * dk) + nk * dij, dij * dk);
                 pm = p0;
                 theta[id] = th;
-                if (i == 0 || j == 0 || k == 0 || i == g.nx - 1 || j == g.ny - 1 || k == g.nz - 1) {
+                if (xy_edge || k == 0 || k == g.nz - 1) {
                     // first ghost layer of theta: wrap on periodic axes, else the nearest interior value (R-12)
                     const int cc[3] = {i, j, k};
                     const int n[3] = {g.nx, g.ny, g.nz};
@@ -260,7 +286,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
                 const double *q = sp + a * FLD;
                 gr[a][0] = xin ? d1_int<ORDER>(q, 1) : d1_line<ORDER>(q, 1, i, g.nx, 0);
                 gr[a][1] = yin ? d1_int<ORDER>(q, BXW) : d1_line<ORDER>(q, BXW, j, g.ny, 0);
-                gr[a][2] = d1_win<ORDER>(w[a], k, g.nz, g.periodic[2]);
+                gr[a][2] = zin ? d1_win<ORDER>(w[a], H, 2 * H + 1, 1) : d1_win<ORDER>(w[a], k, g.nz, 0);
             }
             if (!hoist) {
 #pragma unroll
@@ -275,7 +301,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
                 gz[a] = m[0][2] * gr[a][0] + m[1][2] * gr[a][1] + m[2][2] * gr[a][2];
             }
             const double T = w[0][H], u = w[1][H], v = w[2][H], ww = w[3][H];
-            const double mu0 = fast_div_pos((1.0 + gs.suth) * (T * sqrt(T)), T + gs.suth);  // eq. 15
+            const double mu0 = fast_div_pos((1.0 + gs.suth) * (T * fast_sqrt_pos(T)), T + gs.suth);  // eq. 15
             const double mu = mu0 * gs.invRe, kc = mu0 * gs.kfac;              // eq. 14
             const double div = gx[1] + gy[2] + gz[3];
             const double txx = mu * (2.0 * gx[1] - (2.0 / 3.0) * div);         // eq. 13
@@ -285,20 +311,19 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
             const double thx = u * txx + v * txy + ww * txz + kc * gx[0];      // eq. 12 (R-2)
             const double thy = u * txy + v * tyy + ww * tyz + kc * gy[0];
             const double thz = u * txz + v * tyz + ww * tzz + kc * gz[0];
-            const int c[3] = {i, j, k}, n[3] = {g.nx, g.ny, g.nz};
-            const long long st[3] = {1, g.sy, g.sz};
+            // offset of the periodic image of this point beyond the faces of each direction's own axis (0: none)
+            const long long imz = !g.periodic[2] ? 0 : k < H ? g.nz * g.sz : k >= g.nz - H ? -(g.nz * g.sz) : 0;
+            const long long imo[3] = {imx, imy, imz};
+            double *F = Fp;                                                     // field 4 d + r of this point
 #pragma unroll
             for (int d = 0; d < 3; ++d) {                                       // eq. 9-11
                 const double dx = m[d][0] * iJ, dy = m[d][1] * iJ, dz = m[d][2] * iJ;
-                const double f0 = dx * txx + dy * txy + dz * txz, f1 = dx * txy + dy * tyy + dz * tyz;
-                const double f2 = dx * txz + dy * tyz + dz * tzz, f3 = dx * thx + dy * thy + dz * thz;
-                double *F = Fv + (4 * d) * g.np;
-                __stcs(F + id, f0); __stcs(F + g.np + id, f1); __stcs(F + 2 * g.np + id, f2); __stcs(F + 3 * g.np + id, f3);
-                if (g.periodic[d]) {  // images beyond the faces of this direction's own axis
-                    long long im = -1;
-                    if (c[d] < H) im = id + n[d] * st[d];
-                    else if (c[d] >= n[d] - H) im = id - n[d] * st[d];
-                    if (im >= 0) { F[im] = f0; F[g.np + im] = f1; F[2 * g.np + im] = f2; F[3 * g.np + im] = f3; }
+                const double f[4] = {dx * txx + dy * txy + dz * txz, dx * txy + dy * tyy + dz * tyz,
+                                     dx * txz + dy * tyz + dz * tzz, dx * thx + dy * thy + dz * thz};
+#pragma unroll
+                for (int r = 0; r < 4; ++r, F += g.np) {
+                    __stcs(F, f[r]);
+                    if (imo[d] != 0) F[imo[d]] = f[r];
                 }
             }
         }
@@ -307,7 +332,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
         if (k + H + 1 <= last) {
             const int sc = (k + H + 1 - k0) % VF_NST;
             tma::mbar_wait(&bars[sc], ((k + H + 1 - k0) / VF_NST) & 1);
-            convert_plane<ORDER>(gs, ring + sc * VF_STAGE, tid);
+            convert_plane<ORDER>(gs, ring + sc * VF_STAGE, slots);
         }
         __syncthreads();
         if (tid == 0 && k + VF_NST <= last) issue(k + VF_NST);
