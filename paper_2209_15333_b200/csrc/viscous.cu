@@ -231,8 +231,8 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
     long long id = (long long)(k0 + OCFD_NG) * g.sz + (long long)jp * g.sy + ip;   // this thread's point of plane k
     int sk = 0;                                                                    // ring stage of plane k
     // periodic images in x and y: fixed per thread
-    const long long imx = !g.periodic[0] ? 0 : i < H ? g.nx : i >= g.nx - H ? -g.nx : 0;
-    const long long imy = !g.periodic[1] ? 0 : j < H ? g.ny * g.sy : j >= g.ny - H ? -(g.ny * g.sy) : 0;
+    const int imx = !g.periodic[0] ? 0 : i < H ? 1 : i >= g.nx - H ? -1 : 0;
+    const int imy = !g.periodic[1] ? 0 : j < H ? 1 : j >= g.ny - H ? -1 : 0;
     double *Fp = Fv + id;
     const bool xy_edge = i == 0 || j == 0 || i == g.nx - 1 || j == g.ny - 1;   // touches a face in x or y (theta ghosts)
     for (int k = k0; k < k1; ++k, id += g.sz, Fp += g.sz, sk = sk + 1 == VF_NST ? 0 : sk + 1) {
@@ -311,19 +311,20 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
             const double thx = u * txx + v * txy + ww * txz + kc * gx[0];      // eq. 12 (R-2)
             const double thy = u * txy + v * tyy + ww * tyz + kc * gy[0];
             const double thz = u * txz + v * tyz + ww * tzz + kc * gz[0];
-            // offset of the periodic image of this point beyond the faces of each direction's own axis (0: none)
-            const long long imz = !g.periodic[2] ? 0 : k < H ? g.nz * g.sz : k >= g.nz - H ? -(g.nz * g.sz) : 0;
-            const long long imo[3] = {imx, imy, imz};
-            double *F = Fp;                                                     // field 4 d + r of this point
+            // periodic image of this point beyond the faces of each direction's own axis: +1 / -1 period, 0 = none
+            const int imz = !g.periodic[2] ? 0 : k < H ? 1 : k >= g.nz - H ? -1 : 0;
+            const int ims[3] = {imx, imy, imz};
+            const long long period[3] = {g.nx, (long long)g.ny * g.sy, (long long)g.nz * g.sz};
+            double *F = Fp;                                                     // field 4 d of this point
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {                                       // eq. 9-11
+            for (int d = 0; d < 3; ++d, F += 4 * g.np) {                        // eq. 9-11
                 const double dx = m[d][0] * iJ, dy = m[d][1] * iJ, dz = m[d][2] * iJ;
-                const double f[4] = {dx * txx + dy * txy + dz * txz, dx * txy + dy * tyy + dz * tyz,
-                                     dx * txz + dy * tyz + dz * tzz, dx * thx + dy * thy + dz * thz};
-#pragma unroll
-                for (int r = 0; r < 4; ++r, F += g.np) {
-                    __stcs(F, f[r]);
-                    if (imo[d] != 0) F[imo[d]] = f[r];
+                const double f0 = dx * txx + dy * txy + dz * txz, f1 = dx * txy + dy * tyy + dz * tyz;
+                const double f2 = dx * txz + dy * tyz + dz * tzz, f3 = dx * thx + dy * thy + dz * thz;
+                __stcs(F, f0); __stcs(F + g.np, f1); __stcs(F + 2 * g.np, f2); __stcs(F + 3 * g.np, f3);
+                if (ims[d] != 0) {
+                    double *G = F + (ims[d] > 0 ? period[d] : -period[d]);
+                    G[0] = f0; G[g.np] = f1; G[2 * g.np] = f2; G[3 * g.np] = f3;
                 }
             }
         }
