@@ -6,8 +6,9 @@
 // A CTA owns MAC = 32 pencils (32 consecutive x; for the x sweep 32 consecutive y lines) of one cross index and walks
 // along the sweep direction through the padded rows of its segment in chunks of MR = 4 rows.  Per chunk c:
 //   TMA      the state of the chunk (the five conserved fields as ONE box; theta if hybrid; on curvilinear grids the
-//            metric tables k, sigma and J) arrives in a ring of MNST = 3 stages, requested three chunks ahead by one
-//            thread of the warp that has no phase-A work (one mbarrier per stage);
+//            metric tables k, sigma and J as one more box) arrives in a ring of 4 (curvilinear) or 6 stages, requested
+//            as many chunks ahead as the ring allows by one thread of the warp that has no phase-A work (one mbarrier
+//            per stage);
 //   phase A  one thread per point of the chunk: u, v, w, c from the conserved variables, then the split fluxes
 //            f+-[5] -> shared memory (double-buffered).  Each point is split exactly once per sweep (no halo
 //            recomputation) and neither the primitives nor f+- ever reach HBM (the paper materialises f+-, L549);
@@ -28,14 +29,25 @@ namespace {
 
 constexpr int MAC = 32;             // pencils per CTA (consecutive x)
 constexpr int MR = 4;               // rows per chunk
-constexpr int MNST = 3;             // input stages
 constexpr int MPTS = MAC * MR;      // points per chunk
 constexpr int MNT = 5 * MAC;        // threads: one walker per (pencil, component)
-constexpr int MSTG = 10 * MPTS;     // doubles per input stage: U[5], theta, then k1, k2, k3, sigma (curvilinear)
-constexpr int MNJ = 4;              // slots of the J ring (curvilinear): J of chunk c is used while chunk c+1 is pushed
+// Input ring of one grid kind: a stage holds U[5], theta and, on curvilinear grids, the metric box k1, k2, k3, sigma, J
+// of one chunk; as many stages as three CTAs per SM leave room for (the sweeps wait on HBM latency: with 3 stages the
+// y / z sweeps of a 256^3 box ran at 0.83 of the HBM peak, with 4 at 0.92).
+template <int KIND, int DIR>
+struct MRing {
+    static constexpr int NF = KIND == OCFD_GRID_CURVILINEAR ? 11 : 6;   // fields per stage
+    static constexpr int STG = NF * MPTS;                               // doubles per stage
+    static constexpr int NST = KIND == OCFD_GRID_CURVILINEAR ? 4 : 6;   // stages
+    // chunks requested ahead.  Curvilinear x sweep: one less than the stages, so that the stage of chunk c-1 still holds
+    // its J when phase B of chunk c needs it (the y and z sweeps carry that J in registers instead and use every stage;
+    // the x sweep, which keeps its four outputs of a chunk in registers as well, measured slower that way)
+    static constexpr int PF = KIND == OCFD_GRID_CURVILINEAR && DIR == 0 ? NST - 1 : NST;
+    static constexpr size_t SMEM =
+        sizeof(double) * (size_t)(NST * STG + 2 * 10 * MPTS + 2 * 5 * MPTS) + 8 * NST + 2 * 4 * MAC;
+    static_assert(3 * (SMEM + 1024) <= 233472, "three CTAs per SM");
+};
 constexpr int MTMA = MPTS;          // the thread that issues every TMA operation: lane 0 of the warp without phase-A work
-constexpr size_t M_SMEM =
-    sizeof(double) * (size_t)(MNST * MSTG + MNJ * MPTS + 2 * 10 * MPTS + 2 * 5 * MPTS) + 8 * MNST + 2 * 4 * MAC;
 static_assert(MPTS <= MNT && (MPTS * 8) % 128 == 0, "chunk shape");
 
 // J along one pencil of the sweep: at(g, i0, e) = J at padded row i0 + e
@@ -73,18 +85,18 @@ struct JRow {
 // shared arrays keep the box order (x fastest), the split fluxes are stored with an XOR swizzle of the pencil index so
 // that both the point-wise phase and the walkers are free of bank conflicts, and the output tile is written as two
 // 16-byte stores per walker and leaves by a TMA store (the x sweep writes dU, y and z accumulate).
-// Occupancy: 3 CTAs per SM (128 registers, 65 KB of shared memory each): the hybrid scheme's three code paths need the
+// Occupancy: 3 CTAs per SM (128 registers, 74 KB of shared memory each): the hybrid scheme's three code paths need the
 // 128 registers to keep the unrolled linear path free of spills (measured: 3.8 ms against 4.5 ms per sweep on config 5).
 template <int KIND, int SCHEME, int DIR>
 __global__ void __launch_bounds__(MNT, 3)
     k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_U,
                      const __grid_constant__ CUtensorMap tm_th,
                      const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_met,
-                     const __grid_constant__ CUtensorMap tm_metJ, const int mfull, const int seglen) {
+                     const int mfull, const int seglen) {
+    constexpr int MNST = MRing<KIND, DIR>::NST, MSTG = MRing<KIND, DIR>::STG, MPF = MRing<KIND, DIR>::PF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double *sIn = reinterpret_cast<double *>(smem_raw);   // [MNST][10][MR][MAC]
-    double *sJ = sIn + MNST * MSTG;                       // [MNJ][MR][MAC]
-    double *sF = sJ + MNJ * MPTS;                         // [2][10][MR][MAC]: f+ (0..4), f- (5..9) of chunk c in buffer c % 2
+    double *sIn = reinterpret_cast<double *>(smem_raw);   // [MNST][NF][MR][MAC]
+    double *sF = sIn + MNST * MSTG;                       // [2][10][MR][MAC]: f+ (0..4), f- (5..9) of chunk c in buffer c % 2
     double *sO = sF + 2 * 10 * MPTS;                      // [2][5][MR][MAC] output tiles
     uint64_t *bars = reinterpret_cast<uint64_t *>(sO + 2 * 5 * MPTS);
     unsigned char *sFl = reinterpret_cast<unsigned char *>(bars + MNST);   // [2][MAC][MR] scheme flags pf of chunk c % 2
@@ -116,7 +128,6 @@ __global__ void __launch_bounds__(MNT, 3)
             // z-extruded tables are a few planes that every cross index reads again: ask the L2 to keep them
             const uint64_t keep = tma::policy_evict_last();
             tma::load4_hint(dst + 6 * MPTS, &tm_met, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 0, keep);
-            tma::load4_hint(sJ + (lc % MNJ) * MPTS, &tm_metJ, &bars[s], DIR == 0 ? c1 : c0, DIR == 0 ? c0 : c1, m2, 4, keep);
         }
         tma::load4(dst, &tm_U, &bars[s], c0, c1, c2, 0);
         if (SCHEME == OCFD_HYBRID) tma::load4(dst + 5 * MPTS, &tm_th, &bars[s], c0, c1, c2, 0);
@@ -127,7 +138,9 @@ __global__ void __launch_bounds__(MNT, 3)
         tma::fence_barrier_init();
         issue(0);
         if (nch > 1) issue(1);
-        if (nch > 2) issue(2);
+#pragma unroll
+        for (int q = 2; q < MPF; ++q)
+            if (nch > q) issue(q);
     }
 
     // phase A role: point (row pr, pencil pa) of every chunk; walker role: pencil wa, component wm
@@ -146,6 +159,7 @@ __global__ void __launch_bounds__(MNT, 3)
 #pragma unroll
     for (int e = 0; e < 8; ++e) Wp[e] = Wm[e] = 0.0;
     double hprev = 0.0;
+    double Jnext[MR] = {0.0, 0.0, 0.0, 0.0};   // curvilinear: J of the rows of the chunk whose phase B ran last (see phase B)
     unsigned pprev = 0;     // packed scheme flags pf(r) of the previous chunk's rows, 2 bits per row (hybrid)
     __syncthreads();        // barriers initialised before anyone polls them
 
@@ -206,9 +220,21 @@ __global__ void __launch_bounds__(MNT, 3)
 #pragma unroll
             for (int e = 0; e < MR; ++e) Jw[e] = jrow.at(g, i0, e);
         } else {
-            const double *jp = sJ + ((lc + MNJ - 1) % MNJ) * MPTS;   // arrived with chunk c-1 (rows r0-4 .. r0-1)
+            // J of rows r0-4 .. r0-1 arrived with chunk c-1, whose stage is being refilled by now: this walker took it
+            // into registers during its previous phase B, and now takes the J of this chunk's rows for the next one
+            // (the stage of chunk c is intact until the barrier that ends this interval)
+            if (DIR == 0) {   // (x sweep: straight from the stage of chunk c-1, see MRing::PF)
+                const double *jp = sIn + ((lc + MNST - 1) % MNST) * MSTG + 10 * MPTS;
 #pragma unroll
-            for (int e = 0; e < MR; ++e) Jw[e] = jp[(mfull ? e * MAC : 0) + wa];
+                for (int e = 0; e < MR; ++e) Jw[e] = jp[e * MAC + wa];
+            } else {
+                const double *jp = sIn + (lc % MNST) * MSTG + 6 * MPTS + 4 * (mfull ? MPTS : MAC);
+#pragma unroll
+                for (int e = 0; e < MR; ++e) {
+                    Jw[e] = Jnext[e];
+                    Jnext[e] = jp[(mfull ? e * MAC : 0) + wa];
+                }
+            }
         }
         double *so = sO + PH * 5 * MPTS + wm * MPTS + (DIR == 0 ? wa * MR : wa);
         const double *fpn = sF + PH * 10 * MPTS + wm * MPTS, *fmn = fpn + 5 * MPTS;
@@ -289,8 +315,8 @@ __global__ void __launch_bounds__(MNT, 3)
 
     // One CTA barrier per chunk: between two barriers the CTA runs phase A of chunk c+1 and phase B of chunk c (the
     // split fluxes are double-buffered), so the warp that has no phase-A work and the warps that finish early always
-    // find work of the other kind.  After the barrier: the output tile of chunk c leaves, and the boxes of chunk c+3
-    // are requested into the stage of chunk c (phase A of chunk c+1 has read its last theta row).
+    // find work of the other kind.  After the barrier: the output tile of chunk c leaves, and the boxes of chunk
+    // c + MNST are requested into the stage of chunk c (phase A of chunk c+1 has read its last theta row).
     auto interval = [&](const int lc, auto ph) {
         constexpr int PH = decltype(ph)::value;
         if (lc + 1 < nch) phaseA(lc + 1);
@@ -307,7 +333,7 @@ __global__ void __launch_bounds__(MNT, 3)
                 else tma::reduce_add4(&tm_out, sO + PH * 5 * MPTS, a0, DIR == 1 ? o : cross, DIR == 2 ? o : cross, 0);
                 tma::store_commit();
             }
-            if (lc + 3 < nch) issue(lc + 3);
+            if (lc + MPF < nch) issue(lc + MPF);
         }
     };
     phaseA(0);
@@ -322,6 +348,7 @@ __global__ void __launch_bounds__(MNT, 3)
 template <int KIND, int SCHEME, int DIR>
 ocfd_status launch_march(ocfd_ctx *c) {
     const GridDesc &g = c->g;
+    constexpr size_t M_SMEM = MRing<KIND, DIR>::SMEM;
     if (!ocfd_smem_optin(c, (const void *)k_inviscid_march<KIND, SCHEME, DIR>, M_SMEM)) return OCFD_ECUDA;
     const int ncross = DIR == 2 ? g.ny : g.nz;
     if (ncross > 65535) return OCFD_EINVAL;
@@ -340,7 +367,7 @@ ocfd_status launch_march(ocfd_ctx *c) {
     const MarchMaps &M = c->march;
     const int mfull = DIR != 2 || g.msk != 0;
     k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.U[DIR], M.th[DIR], M.out[DIR],
-                                                                        M.met[DIR], M.metJ[DIR], mfull, seglen);
+                                                                        M.met[DIR], mfull, seglen);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
 }
@@ -374,18 +401,16 @@ bool encode_march_maps(ocfd_ctx *c, const double *U, double *dU) {
                 // the derived metric table of this direction: [5][planes][nyp][nxp], one plane if z-extruded
                 const long long mdim[4] = {g.nxp, g.nyp, g.msk ? g.nzp : 1, 5};
                 const int mz = d == 2 && g.msk ? MR : 1;
-                const int m4[4] = {bx, by, mz, 4}, m1[4] = {bx, by, mz, 1};
+                const int m5[4] = {bx, by, mz, 5};   // k1, k2, k3, sigma, J as one box
                 if (d == 0) {   // y-contiguous copy [5][planes][nxp][nypT]: boxes of 4 rows of 32 lines
                     const long long tdim[4] = {g.nyp, g.nxp, g.msk ? g.nzp : 1, 5};
-                    const int t4[4] = {MAC, MR, 1, 4}, t1[4] = {MAC, MR, 1, 1};
-                    if (!ocfd_tma_encode(&M.met[d], g.atabT, tdim, g.nypT, (long long)g.nxp * g.nypT, g.atabT_fs, t4)) return false;
-                    if (!ocfd_tma_encode(&M.metJ[d], g.atabT, tdim, g.nypT, (long long)g.nxp * g.nypT, g.atabT_fs, t1)) return false;
+                    const int t5[4] = {MAC, MR, 1, 5};
+                    if (!ocfd_tma_encode(&M.met[d], g.atabT, tdim, g.nypT, (long long)g.nxp * g.nypT, g.atabT_fs, t5)) return false;
                 } else {
-                    if (!ocfd_tma_encode(&M.met[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m4)) return false;
-                    if (!ocfd_tma_encode(&M.metJ[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m1)) return false;
+                    if (!ocfd_tma_encode(&M.met[d], g.atab[d], mdim, g.sy, g.sz, g.atab_fs, m5)) return false;
                 }
             } else {   // unused, but the kernel takes the parameters
-                M.met[d] = M.metJ[d] = CUtensorMap();
+                M.met[d] = CUtensorMap();
             }
             if (!ocfd_tma_encode(&M.th[d], c->theta, full1, g.sy, g.sz, g.np, b1, d == 0)) return false;
         }

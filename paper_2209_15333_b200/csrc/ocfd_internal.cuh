@@ -70,7 +70,7 @@ struct InvMaps {
 struct MarchMaps {
     const double *Up, *dUp;
     bool ready;
-    CUtensorMap U[3], th[3], out[3], met[3], metJ[3];
+    CUtensorMap U[3], th[3], out[3], met[3];
 };
 // ... of the fused x-y sweep (inviscid_xy.cu)
 struct XYMaps {
