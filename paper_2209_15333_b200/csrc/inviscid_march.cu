@@ -34,11 +34,12 @@ constexpr int MNT = 5 * MAC;        // threads: one walker per (pencil, componen
 // Input ring of one grid kind: a stage holds U[5], theta and, on curvilinear grids, the metric box k1, k2, k3, sigma, J
 // of one chunk; as many stages as three CTAs per SM leave room for (the sweeps wait on HBM latency: with 3 stages the
 // y / z sweeps of a 256^3 box ran at 0.83 of the HBM peak, with 4 at 0.92).
-template <int KIND, int DIR>
+// MFULL = 0: the z sweep over a z-extruded curvilinear map, whose metric box is one row for the whole chunk.
+template <int KIND, int DIR, bool MFULL>
 struct MRing {
-    static constexpr int NF = KIND == OCFD_GRID_CURVILINEAR ? 11 : 6;   // fields per stage
-    static constexpr int STG = NF * MPTS;                               // doubles per stage
-    static constexpr int NST = KIND == OCFD_GRID_CURVILINEAR ? 4 : 6;   // stages
+    static constexpr int MBOX = KIND != OCFD_GRID_CURVILINEAR ? 0 : 5 * (MFULL ? MPTS : MAC);   // doubles of the metric box
+    static constexpr int STG = 6 * MPTS + MBOX;                          // doubles per stage
+    static constexpr int NST = KIND != OCFD_GRID_CURVILINEAR ? 6 : MFULL ? 4 : 6;   // stages
     // chunks requested ahead.  Curvilinear x sweep: one less than the stages, so that the stage of chunk c-1 still holds
     // its J when phase B of chunk c needs it (the y and z sweeps carry that J in registers instead and use every stage;
     // the x sweep, which keeps its four outputs of a chunk in registers as well, measured slower that way)
@@ -87,13 +88,14 @@ struct JRow {
 // 16-byte stores per walker and leaves by a TMA store (the x sweep writes dU, y and z accumulate).
 // Occupancy: 3 CTAs per SM (128 registers, 74 KB of shared memory each): the hybrid scheme's three code paths need the
 // 128 registers to keep the unrolled linear path free of spills (measured: 3.8 ms against 4.5 ms per sweep on config 5).
-template <int KIND, int SCHEME, int DIR>
+template <int KIND, int SCHEME, int DIR, bool MFULL>
 __global__ void __launch_bounds__(MNT, 3)
     k_inviscid_march(const GridDesc g, const GasDesc gs, const __grid_constant__ CUtensorMap tm_U,
                      const __grid_constant__ CUtensorMap tm_th,
                      const __grid_constant__ CUtensorMap tm_out, const __grid_constant__ CUtensorMap tm_met,
-                     const int mfull, const int seglen) {
-    constexpr int MNST = MRing<KIND, DIR>::NST, MSTG = MRing<KIND, DIR>::STG, MPF = MRing<KIND, DIR>::PF;
+                     const int seglen) {
+    constexpr bool mfull = MFULL;
+    constexpr int MNST = MRing<KIND, DIR, MFULL>::NST, MSTG = MRing<KIND, DIR, MFULL>::STG, MPF = MRing<KIND, DIR, MFULL>::PF;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *sIn = reinterpret_cast<double *>(smem_raw);   // [MNST][NF][MR][MAC]
     double *sF = sIn + MNST * MSTG;                       // [2][10][MR][MAC]: f+ (0..4), f- (5..9) of chunk c in buffer c % 2
@@ -345,11 +347,11 @@ __global__ void __launch_bounds__(MNT, 3)
     if (tid == MTMA) tma::store_wait_all<0>();
 }
 
-template <int KIND, int SCHEME, int DIR>
-ocfd_status launch_march(ocfd_ctx *c) {
+template <int KIND, int SCHEME, int DIR, bool MFULL>
+ocfd_status launch_march_m(ocfd_ctx *c) {
     const GridDesc &g = c->g;
-    constexpr size_t M_SMEM = MRing<KIND, DIR>::SMEM;
-    if (!ocfd_smem_optin(c, (const void *)k_inviscid_march<KIND, SCHEME, DIR>, M_SMEM)) return OCFD_ECUDA;
+    constexpr size_t M_SMEM = MRing<KIND, DIR, MFULL>::SMEM;
+    if (!ocfd_smem_optin(c, (const void *)k_inviscid_march<KIND, SCHEME, DIR, MFULL>, M_SMEM)) return OCFD_ECUDA;
     const int ncross = DIR == 2 ? g.ny : g.nz;
     if (ncross > 65535) return OCFD_EINVAL;
     const int nd = DIR == 0 ? g.nx : DIR == 1 ? g.ny : g.nz, ntile = ((DIR == 0 ? g.ny : g.nx) + MAC - 1) / MAC;
@@ -365,11 +367,18 @@ ocfd_status launch_march(ocfd_ctx *c) {
     dim3 grd(ntile, ncross, nseg);
     OCFD_T0(c, K_INV_X + DIR);
     const MarchMaps &M = c->march;
-    const int mfull = DIR != 2 || g.msk != 0;
-    k_inviscid_march<KIND, SCHEME, DIR><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.U[DIR], M.th[DIR], M.out[DIR],
-                                                                        M.met[DIR], mfull, seglen);
+    k_inviscid_march<KIND, SCHEME, DIR, MFULL><<<grd, MNT, M_SMEM, c->stream>>>(g, c->gas, M.U[DIR], M.th[DIR], M.out[DIR],
+                                                                               M.met[DIR], seglen);
     OCFD_CHECK_LAUNCH(c);
     return OCFD_OK;
+}
+
+// the z sweep over a z-extruded curvilinear map has an instance of its own (one metric row per chunk: smaller stages,
+// more of them)
+template <int KIND, int SCHEME, int DIR>
+ocfd_status launch_march(ocfd_ctx *c) {
+    if (KIND == OCFD_GRID_CURVILINEAR && DIR == 2 && c->g.msk == 0) return launch_march_m<KIND, SCHEME, DIR, false>(c);
+    return launch_march_m<KIND, SCHEME, DIR, true>(c);
 }
 
 template <int KIND, int SCHEME>
