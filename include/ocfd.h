@@ -134,6 +134,30 @@ ocfd_status ocfd_rk3_steps_host(ocfd_ctx *ctx, double *U_host, double *U_dev, do
  * the caller sets dt = CFL / Lambda.  Writes one double to host_out and synchronises the stream. */
 ocfd_status ocfd_max_wavespeed(ocfd_ctx *ctx, const double *U, double *host_out);
 
+/* Row a9 for callers that cannot allocate device memory.  Everything else in this header needs a context, and a
+ * context needs a workspace of several fields from the caller; code that must not call cudaMalloc -- a callback inside
+ * an application whose own pool already owns all of HBM, a monitoring hook that may not disturb the allocator, a job
+ * whose memory budget is spent on the flow fields -- cannot supply one.  This call needs neither: pass the same
+ * parameter block a context would get (only nx, ny, nz, ng, grid_kind, metric, metric_plane_stride, dx, dy, dz, gamma,
+ * Ma and stream are used; workspace may be NULL; the block must still be one ocfd_init would accept), the state U
+ * (device pointer, ghosts not read) and a host pointer for the result.  Same value as ocfd_max_wavespeed (a maximum
+ * does not depend on the order it is taken in), NaN for a state with a non-finite wavespeed, and like it the call
+ * returns after the stream has drained.  It calls no cudaMalloc, cudaFree or allocating library routine.
+ *
+ * The reduction's scratch is a fixed array inside the library image: (OCFD_STATIC_WAVESPEED_SLOTS + 32) * 8 bytes =
+ * 512.25 KiB on every GPU that loads the library, held until the process exits.  Limits and rules that follow:
+ *   - ceil(nx / 128) * ny must not exceed OCFD_STATIC_WAVESPEED_SLOTS; a larger grid is refused with OCFD_EWORKSPACE
+ *     and one line on stderr, before anything is launched (use ocfd_max_wavespeed with a context for such grids);
+ *   - all calls on one device share the array.  No call depends on what an earlier one left in it, but two calls that
+ *     run on the same GPU at the same time (from two threads or on two streams) corrupt each other's result: serialise
+ *     them.  Calls made one after the other from one thread are safe, since each returns only when its work is done;
+ *   - the first call on each device also looks up the array's device address (host-side work, no allocation); the
+ *     device the stream belongs to must be current, and that first call should be made before any stream capture.
+ * Errors: OCFD_EINVAL (null pointer, parameters ocfd_init would reject, ny > 65535), OCFD_EWORKSPACE (grid beyond the
+ * limit above), OCFD_EUNSUPPORTED (not an sm_100 device), OCFD_ECUDA. */
+#define OCFD_STATIC_WAVESPEED_SLOTS 65536
+ocfd_status ocfd_max_wavespeed_static(const ocfd_params *p, const double *U, double *host_out);
+
 /* Hybrid-scheme parity report: theta (padded field, interior + the first ghost layer of each face written) and
  * the per-interface scheme flags (0 UD7, 1 WENO7, 2 WENO5): flag_xyz is [3][nz+8][ny+8][nx+8] bytes and
  * flag_xyz[d][point s] is the scheme of interface s+1/2 along direction d, s = -1 .. n-1.  Either output

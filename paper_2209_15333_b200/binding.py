@@ -18,7 +18,8 @@ OCFD_OK = 0
 
 EXPORTS = ["ocfd_workspace_bytes", "ocfd_init", "ocfd_destroy", "ocfd_fill_ghosts", "ocfd_rhs", "ocfd_rk3_step",
            "ocfd_rk3_steps_host", "ocfd_max_wavespeed", "ocfd_debug_sensor", "ocfd_timing", "ocfd_timing_read",
-           "ocfd_kernel_name", "ocfd_sizeof_params", "ocfd_launch_count", "ocfd_strerror", "ocfd_set_tuning"]
+           "ocfd_kernel_name", "ocfd_sizeof_params", "ocfd_launch_count", "ocfd_strerror", "ocfd_set_tuning",
+           "ocfd_max_wavespeed_static"]
 NKERNELS = 10
 
 
@@ -78,6 +79,8 @@ def load():
     L.ocfd_rk3_steps_host.argtypes = [vp, vp, vp, C.c_double, C.c_int]
     L.ocfd_max_wavespeed.restype = C.c_int
     L.ocfd_max_wavespeed.argtypes = [vp, vp, C.POINTER(C.c_double)]
+    L.ocfd_max_wavespeed_static.restype = C.c_int
+    L.ocfd_max_wavespeed_static.argtypes = [pp, vp, C.POINTER(C.c_double)]
     L.ocfd_debug_sensor.restype = C.c_int
     L.ocfd_debug_sensor.argtypes = [vp, vp, vp, vp]
     L.ocfd_launch_count.restype = C.c_longlong
@@ -128,6 +131,15 @@ def params_from_case(case):
         P.bc[f] = BCS[case.bc[f]]
         P.T_wall[f] = case.T_wall[f]
     return P
+
+
+def max_wavespeed_static(P, U_ptr):
+    """ocfd_max_wavespeed_static: Lambda of the state at device address `U_ptr` for the grid and gas an OcfdParams `P`
+    describes, with no context and no workspace.  For callers that may not allocate device memory; the scratch is a
+    fixed array inside the library (limits and sharing rules: include/ocfd.h)."""
+    out = C.c_double(0.0)
+    _check(load().ocfd_max_wavespeed_static(C.byref(P), U_ptr, C.byref(out)))
+    return out.value
 
 
 class Solver:

@@ -76,3 +76,18 @@ def test_product_path_never_imports_the_oracle():
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in txt.replace("test oracle", "").replace("the oracle", "").replace("CPU oracle", "") \
                     or f == "workloads.py", f
+
+
+def test_static_wavespeed_size_limit_is_checked_on_the_host(B):
+    """ocfd_max_wavespeed_static (the entry point for callers that cannot allocate device memory) refuses a grid beyond
+    its fixed scratch array, and bad arguments, before it touches the GPU: none is needed to see that."""
+    L = B.load()
+    P = B.params_from_case(W.tgv(16))
+    P.nx, P.ny, P.nz = 1024, 8200, 16                      # ceil(1024/128) * 8200 = 65600 > 65536 slots
+    never_read = (C.c_double * 8)()
+    out = C.c_double(-1.0)
+    assert L.ocfd_max_wavespeed_static(C.byref(P), never_read, C.byref(out)) == -2
+    P.nx = 6
+    assert L.ocfd_max_wavespeed_static(C.byref(P), never_read, C.byref(out)) == -1
+    assert L.ocfd_max_wavespeed_static(C.byref(B.params_from_case(W.tgv(16))), None, C.byref(out)) == -1
+    assert out.value == -1.0
