@@ -104,7 +104,8 @@ def step_both_hybrid(B, Oracle, case, nsteps, band=1e-9, check_flags_every=1, lo
     stages of reach 6) are excluded from the comparison.  At the start of every `check_flags_every`-th step the GPU's
     own decisions (ocfd_debug_sensor) are compared with the oracle's, outside the 1e-12 band of north_star.
 
-    Returns dict(err_all, err_outside, excluded_fraction, near, flag_mismatches, flag_inband, hist0, hist_end)."""
+    Returns dict(err_all, err_outside, err_padded_outside (the same bar over the whole padded array: face ghosts
+    included), excluded_fraction, near, flag_mismatches, flag_inband, hist0, hist_end)."""
     o = Oracle(case)
     U = o.fill_ghosts(case.U0.copy())
     dt = case.cfl / o.max_wavespeed(U)
@@ -156,7 +157,16 @@ def step_both_hybrid(B, Oracle, case, nsteps, band=1e-9, check_flags_every=1, lo
         err_out = max(np.abs(gi[m] - ui[m])[keep].max() / den[m] for m in range(5))
     else:
         err_out = float("nan")
-    res = dict(err_all=float(err_all), err_outside=float(err_out), excluded_fraction=float(excl.mean()),
+    # the whole padded array as well: both sides leave the face ghosts filled by the last ghost fill of the step (from
+    # two different buffers on the GPU side, ocfd_rk3_step rotates them); edges and corners are written by neither and
+    # still hold the initial values.  A ghost point counts as excluded if the interior point nearest to it is.
+    keep_p = np.pad(keep, NG, mode="edge")
+    if keep_p.any():
+        err_pad = max(np.abs(got[m] - U[m])[keep_p].max() / max(np.abs(U[m]).max(), floor) for m in range(5))
+    else:
+        err_pad = float("nan")
+    res = dict(err_all=float(err_all), err_outside=float(err_out), err_padded_outside=float(err_pad),
+               excluded_fraction=float(excl.mean()),
                near=near_total, flag_mismatches=bad_total, flag_inband=inband_total,
                hist0=None if hist0 is None else hist0.tolist(), hist_end=None if hist_end is None else hist_end.tolist(),
                finite=bool(np.isfinite(got).all()))

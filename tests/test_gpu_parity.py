@@ -95,12 +95,76 @@ def test_rhs_parity_smooth_periodic(B, Oracle, grid, scheme):
     assert err.max() <= TOL_RHS, err
 
 
-@pytest.mark.parametrize("scheme", ["ud7", "weno7"])
+@pytest.mark.parametrize("scheme", ["ud7", "weno7", "hybrid"])
 def test_rhs_parity_inviscid_only_and_sw_eps(B, Oracle, scheme):
     case = W.smooth_periodic(58, 21, 41, grid="wavy", scheme=scheme, inviscid=True, seed=5)
     case.sw_eps = 0.02
     got, ref, U = run_rhs_both(B, Oracle, case)
     assert rel_linf(got, ref, U).max() <= TOL_RHS
+
+
+def shocked_box(nx, ny, nz, grid, scheme, aperiodic, seed=9):
+    """Inviscid case with steep fronts on any of the smooth_periodic grids (the recipe of W.shocked_periodic on a
+    non-cubic, optionally curvilinear box), periodic or with extrapolation on all six faces.  Inputs only."""
+    case = W.smooth_periodic(nx, ny, nz, seed=seed, scheme=scheme, Ma=1.2, amp=0.15, inviscid=True, grid=grid)
+    KK, JJ, II = np.meshgrid(np.arange(-NG, nz + NG), np.arange(-NG, ny + NG), np.arange(-NG, nx + NG), indexing="ij")
+    a, b, c = 2 * np.pi * II / nx, 2 * np.pi * JJ / ny, 2 * np.pi * KK / nz
+    front = 0.5 * (1.0 + np.tanh(5.0 * np.sin(a + 0.7 * np.sin(b)) * np.cos(c + 0.3)))
+    fac = 1.0 + 1.5 * front
+    U = case.U0.copy()
+    U[:4] *= fac
+    U[4] *= fac * (1.0 + 0.8 * front)
+    case.U0 = np.ascontiguousarray(U)
+    case.theta1, case.theta2 = 0.02, 0.1
+    if aperiodic:
+        case.bc = ["outflow"] * 6
+    case.name = f"shocked_box_{grid}_{scheme}_{'open' if aperiodic else 'periodic'}"
+    return case
+
+
+@pytest.mark.parametrize("which", ["uniform-periodic", "wavy-open", "stretched-open"])
+def test_inviscid_hybrid_standalone_sensor_flags_and_rhs(B, Oracle, which):
+    """Runs without viscous terms take theta from the stand-alone sensor kernel (with them it is part of viscous
+    pass 1): theta on the interior AND on the first ghost layer of every face (copy rule on aperiodic faces, R-12),
+    the per-interface decisions, and the hybrid RHS built on them, against the CPU reference."""
+    grid, ends = which.split("-")
+    case = shocked_box(70, 45, 23, grid, "hybrid", ends == "open")
+    o = Oracle(case)
+    U = o.fill_ghosts(case.U0.copy())
+    bad, near, total, hist = flag_report(B, Oracle, case, U)
+    print(f"{case.name}: {total} interfaces, {near} within 1e-12 of a threshold, {bad} mismatches, "
+          f"UD7/WENO7/WENO5 = {hist.tolist()}")
+    assert bad == 0 and np.all(hist > 0)
+    th_ref = o.sensor(U)
+    s = B.Solver(case)
+    th_gpu = s.debug_sensor(s.to_device(U))[0].cpu().numpy()
+    s.close()
+    I = slice(NG, -NG)
+    for lo, hi in (((NG - 1, I, I), (-NG, I, I)), ((I, NG - 1, I), (I, -NG, I)), ((I, I, NG - 1), (I, I, -NG))):
+        for face in (lo, hi):
+            assert np.abs(th_gpu[face] - th_ref[face]).max() <= 1e-13, (which, face)
+    got, ref, Ui = run_rhs_both(B, Oracle, case)
+    assert rel_linf(got, ref, Ui).max() <= TOL_RHS
+
+
+@pytest.mark.parametrize("which", ["ud7-wavy-periodic", "weno7-wavy-open", "weno5-stretched-open", "hybrid-uniform-periodic",
+                                   "hybrid-wavy-open"])
+def test_inviscid_ten_steps_standalone_update(B, Oracle, which):
+    """Without viscous terms the RK3 stage update is a kernel of its own (with them it is folded into viscous pass 2)
+    working on the rotating state buffers: 10 steps against the CPU reference at the 1e-9 bar, face ghosts included."""
+    from tests.parity_utils import step_both_hybrid
+    scheme, grid, ends = which.split("-")
+    case = shocked_box(46, 30, 20, grid, scheme, ends == "open") if scheme == "hybrid" else \
+        W.smooth_periodic(46, 30, 20, grid=grid, scheme=scheme, inviscid=True, seed=12)
+    if ends == "open":
+        case.bc = ["outflow"] * 6
+    res = step_both_hybrid(B, Oracle, case, 10)
+    assert res["finite"] and res["flag_mismatches"] == 0
+    if res["err_all"] > TOL_100:
+        assert res["near"] > 0 and res["excluded_fraction"] < 1.0 and res["err_outside"] <= TOL_100, res
+    assert res["err_padded_outside"] <= TOL_100, res
+    if scheme == "hybrid":
+        assert res["hist0"][0] > 0 and res["hist0"][1] + res["hist0"][2] > 0
 
 
 def test_rhs_freestream_is_zero_to_roundoff(B, Oracle):
@@ -417,6 +481,23 @@ def test_launch_shape_knobs_change_no_bit(B, which):
         assert bool((Ua == Ub).all()), knobs
 
 
+def test_set_tuning_refuses_what_the_launchers_would_ignore(B):
+    """include/ocfd.h: a zchunk value is 0 (automatic) or at least 8; unknown keys and negative values are errors."""
+    s = B.Solver(W.smooth_periodic(8, 8, 8))
+    for key in ("zchunk_flux", "zchunk_div", "zchunk_sensor"):
+        for v in (1, 7, -1):
+            with pytest.raises(B.OcfdError, match="invalid"):
+                s.set_tuning(key, v)
+        s.set_tuning(key, 8)
+        s.set_tuning(key, 0)
+    for key in ("xy_fused", "zchunk", ""):
+        with pytest.raises(B.OcfdError, match="invalid"):
+            s.set_tuning(key, 1)
+    s.set_tuning("march_seg", 3)
+    s.set_tuning("tile_group", 1)
+    s.close()
+
+
 def test_invalid_parameters_are_refused_without_touching_buffers(B):
     """Argument errors come back as status codes (never exceptions from the library), synchronously."""
     case = W.smooth_periodic(8, 8, 8)
@@ -501,3 +582,4 @@ def test_twenty_steps_with_walls(B, Oracle, which):
     assert res["finite"] and res["flag_mismatches"] == 0
     if res["err_all"] > TOL_100:
         assert res["near"] > 0 and res["excluded_fraction"] < 1.0 and res["err_outside"] <= TOL_100, res
+    assert res["err_padded_outside"] <= TOL_100, res          # face ghosts of the stepped state included
