@@ -127,9 +127,7 @@ def algorithmic(case, flag_hist=None):
     out = {
         "ghost_fill": (0.0, 0.0),
         "shock_sensor": (40.0 + 8.0, 25.0 + prim_flops),      # stand-alone form (runs without viscous terms)
-        # x and y sweeps fused: the state is read once and dU written once for both directions
-        "inviscid_xy": (state + th + 2 * m_inv + 40, 2 * (10 * fl_rec + 5 + 140 + 15) + prim_flops),
-        # one launch per direction (characteristic variables, and the unfused reference): x writes dU, y / z add into it
+        # one launch per direction: x writes dU, y / z add into it
         # (TMA reduce at the L2: dU still crosses HBM in and out)
         "inviscid_x": (state + th + m_inv + 40, inv_flops),
         "inviscid_y": (state + th + m_inv + 80, inv_flops),

@@ -14,7 +14,8 @@
  * (i+4, j+4, k+4).  Edge and corner ghosts are never read nor written by any entry point.
  *
  * Errors: every entry point returns an ocfd_status; argument errors are detected synchronously and leave all
- * buffers untouched; CUDA launch errors map to OCFD_ECUDA.  No global state; several contexts may coexist.
+ * buffers untouched; CUDA launch errors map to OCFD_ECUDA.  No global state (the one exception is the fixed scratch array
+ * of ocfd_max_wavespeed_static, see there); several contexts may coexist.
  * There is no CPU fallback of any kind.
  */
 #ifndef OCFD_H
@@ -165,11 +166,11 @@ ocfd_status ocfd_max_wavespeed_static(const ocfd_params *p, const double *U, dou
 ocfd_status ocfd_debug_sensor(ocfd_ctx *ctx, const double *U, double *theta, unsigned char *flag_xyz);
 
 /* Launch-shape knobs of one context, for A/B measurements; they change no result beyond round-off.  Keys:
- * "xy_fused" (0, default: one marching launch per sweep direction; 1: the x and y sweeps run as one kernel, an
- * experiment that is slower on every measured workload), "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a CTA of
+ * "zchunk_flux", "zchunk_div", "zchunk_sensor" (planes a CTA of
  * the viscous passes / the stand-alone sensor marches; 0 automatic, else >= 8), "march_seg" (segments a pencil of the
  * marching sweeps is cut into; 0 automatic), "tile_group" (tiles per column group in the CTA numbering of the viscous
- * passes; 0 = 16, a value >= the tiles per row gives the plain x-fastest order).  Unknown key or negative value: OCFD_EINVAL. */
+ * passes; 0 = 16, a value >= the tiles per row gives the plain x-fastest order).  Unknown key, negative value or a
+ * zchunk value between 1 and 7: OCFD_EINVAL. */
 ocfd_status ocfd_set_tuning(ocfd_ctx *ctx, const char *key, int value);
 
 /* sizeof(ocfd_params) as compiled, so that a foreign-language mirror of the struct can check itself. */
@@ -180,7 +181,7 @@ size_t ocfd_sizeof_params(void);
  * synchronises the stream, adds up the elapsed milliseconds and launch counts per class since the last read
  * into ms[OCFD_NKERNELS] / launches[OCFD_NKERNELS] (host arrays) and clears the record.  Class names:
  * ocfd_kernel_name(id), id = 0 .. OCFD_NKERNELS-1. */
-#define OCFD_NKERNELS 10
+#define OCFD_NKERNELS 9
 ocfd_status ocfd_timing(ocfd_ctx *ctx, int enable);
 ocfd_status ocfd_timing_read(ocfd_ctx *ctx, double *ms, long long *launches);
 const char *ocfd_kernel_name(int id);

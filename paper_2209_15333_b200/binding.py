@@ -20,7 +20,7 @@ EXPORTS = ["ocfd_workspace_bytes", "ocfd_init", "ocfd_destroy", "ocfd_fill_ghost
            "ocfd_rk3_steps_host", "ocfd_max_wavespeed", "ocfd_debug_sensor", "ocfd_timing", "ocfd_timing_read",
            "ocfd_kernel_name", "ocfd_sizeof_params", "ocfd_launch_count", "ocfd_strerror", "ocfd_set_tuning",
            "ocfd_max_wavespeed_static"]
-NKERNELS = 10
+NKERNELS = 9
 
 
 class OcfdParams(C.Structure):

@@ -13,8 +13,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libocfd_b200.so")
-SOURCES = ["api.cu", "ghost.cu", "prim.cu", "metrics.cu", "inviscid.cu", "inviscid_march.cu", "inviscid_xy.cu",
-           "viscous.cu", "rk.cu", "wavespeed_static.cu"]
+SOURCES = ["api.cu", "ghost.cu", "prim.cu", "metrics.cu", "inviscid.cu", "inviscid_march.cu", "viscous.cu", "rk.cu",
+           "wavespeed_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 

@@ -103,7 +103,6 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->stream = (cudaStream_t)p->stream;
     c->nsm = nsm;
     c->tune = Tuning();
-    c->tune.xy_fused = 0;
     c->visc_order = p->visc_order == 8 ? 8 : 6;
     GridDesc &g = c->g;
     g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
@@ -155,8 +154,6 @@ ocfd_status ocfd_init(ocfd_ctx **out, const ocfd_params *p) {
     c->inv.Up = c->inv.dUp = nullptr;
     c->march.ready = false;
     c->march.Up = c->march.dUp = nullptr;
-    c->xy.ready = false;
-    c->xy.Up = c->xy.dUp = nullptr;
     c->sens_U = nullptr;
     c->visc.ready = false;
     c->visc.Ufp = c->visc.Up = c->visc.dUp = nullptr;
@@ -281,7 +278,7 @@ ocfd_status ocfd_timing_read(ocfd_ctx *c, double *ms, long long *launches) {
 }
 
 const char *ocfd_kernel_name(int id) {
-    static const char *names[OCFD_NKERNELS] = {"ghost_fill", "shock_sensor", "inviscid_xy", "inviscid_x", "inviscid_y",
+    static const char *names[OCFD_NKERNELS] = {"ghost_fill", "shock_sensor", "inviscid_x", "inviscid_y",
                                                "inviscid_z", "viscous_flux", "viscous_div", "rk3_update", "max_wavespeed"};
     return id >= 0 && id < OCFD_NKERNELS ? names[id] : "?";
 }
@@ -291,8 +288,9 @@ size_t ocfd_sizeof_params(void) { return sizeof(ocfd_params); }
 ocfd_status ocfd_set_tuning(ocfd_ctx *c, const char *key, int value) {
     if (!live(c)) return OCFD_ESTATE;
     if (!key || value < 0) return OCFD_EINVAL;
-    if (!strcmp(key, "xy_fused")) { if (value > 1) return OCFD_EINVAL; c->tune.xy_fused = value; }
-    else if (!strcmp(key, "zchunk_flux")) c->tune.zchunk_f = value;
+    const bool zchunk = !strncmp(key, "zchunk_", 7);
+    if (zchunk && value > 0 && value < 8) return OCFD_EINVAL;   // the marches need chunks of at least 8 planes
+    if (!strcmp(key, "zchunk_flux")) c->tune.zchunk_f = value;
     else if (!strcmp(key, "zchunk_div")) c->tune.zchunk_d = value;
     else if (!strcmp(key, "zchunk_sensor")) c->tune.zchunk_s = value;
     else if (!strcmp(key, "march_seg")) c->tune.march_seg = value;

@@ -1,7 +1,7 @@
 // Rows a2 + a4 + a5 with the reconstruction in CHARACTERISTIC VARIABLES (ocfd_params.char_recon):
 // primitives from U, Steger-Warming split (eq. 19-29), projection on the eigenvectors of the
 // interface, UD7 / WENO7 / WENO5 reconstruction (eq. 41) and the conservative flux difference, one
-// launch per sweep direction (tile kernel).  The component-wise sweeps are inviscid_xy.cu and inviscid_march.cu.
+// launch per sweep direction (tile kernel).  The component-wise sweeps are inviscid_march.cu.
 //
 // One CTA owns a tile of AC = 16 pencils x OUTS = 24 outputs along the sweep.  The state of the tile plus its 4-point
 // halos (32 points along the sweep) is fetched by two TMA box loads (the five conserved fields as one box; theta for
@@ -390,9 +390,9 @@ bool encode_maps(ocfd_ctx *c, const double *U, double *dU) {
 
 }  // namespace
 
-// dU <- -J sum_d (h_{s+1/2} - h_{s-1/2}).  Component-wise reconstruction: the fused x-y kernel writes dU, the z sweep
-// accumulates by TMA reduce-add (one add per element and kernel, in stream order: bitwise reproducible).  In
-// characteristic variables: the tile kernel, once per direction.
+// dU <- -J sum_d (h_{s+1/2} - h_{s-1/2}).  Component-wise reconstruction: one marching launch per direction; the x sweep
+// writes dU, the y and z sweeps accumulate by TMA reduce-add (one add per element and kernel, in stream order: bitwise
+// reproducible).  In characteristic variables: the tile kernel, once per direction.
 ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU) {
     ocfd_status st;
     if (c->p.char_recon) {
@@ -403,12 +403,7 @@ ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU) {
             default: return launch_kind<OCFD_GRID_CURVILINEAR>(c, U);
         }
     }
-    if (c->tune.xy_fused) {
-        st = launch_inviscid_xy(c, U, dU);
-    } else {   // unfused reference (A/B measurements): x writes, y accumulates
-        if ((st = launch_inviscid_march(c, U, dU, 0)) != OCFD_OK) return st;
-        st = launch_inviscid_march(c, U, dU, 1);
-    }
-    if (st != OCFD_OK) return st;
+    if ((st = launch_inviscid_march(c, U, dU, 0)) != OCFD_OK) return st;
+    if ((st = launch_inviscid_march(c, U, dU, 1)) != OCFD_OK) return st;
     return launch_inviscid_march(c, U, dU, 2);
 }

@@ -1,7 +1,6 @@
 // Rows a2 + a4 + a5 of ONE sweep direction: primitives from U, Steger-Warming split (eq. 19-29),
 // UD7 / WENO7 / WENO5 reconstruction (eq. 41) and the conservative flux difference, as a MARCHING
-// kernel.  It runs the x, y and z sweeps of every run in component-wise variables (ocfd_set_tuning "xy_fused" = 1
-// replaces the x and y launches by the fused kernel of inviscid_xy.cu, an experiment that measured slower).
+// kernel.  It runs the x, y and z sweeps of every run in component-wise variables.
 //
 // A CTA owns MAC = 32 pencils (32 consecutive x; for the x sweep 32 consecutive y lines) of one cross index and walks
 // along the sweep direction through the padded rows of its segment in chunks of MR = 4 rows.  Per chunk c:

@@ -54,7 +54,7 @@ struct GasDesc {
 };
 
 // kernel classes, for ocfd_timing_read / ocfd_kernel_name (K_INV_X + d = the sweep of direction d as its own launch)
-enum { K_GHOST = 0, K_SENSOR, K_INV_XY, K_INV_X, K_INV_Y, K_INV_Z, K_VISC_FLUX, K_VISC_DIV, K_RK, K_WAVE, K_COUNT };
+enum { K_GHOST = 0, K_SENSOR, K_INV_X, K_INV_Y, K_INV_Z, K_VISC_FLUX, K_VISC_DIV, K_RK, K_WAVE, K_COUNT };
 static_assert(K_COUNT == OCFD_NKERNELS, "kernel class count");
 
 struct TimedLaunch { cudaEvent_t a, b; int id; };
@@ -72,12 +72,6 @@ struct MarchMaps {
     bool ready;
     CUtensorMap U[3], th[3], out[3], met[3];
 };
-// ... of the fused x-y sweep (inviscid_xy.cu)
-struct XYMaps {
-    const double *Up, *dUp;
-    bool ready;
-    CUtensorMap U, th, out;
-};
 // ... and of the two viscous passes
 struct ViscMaps {
     const double *Ufp, *Up, *dUp;
@@ -87,7 +81,6 @@ struct ViscMaps {
 
 // Tuning knobs of one context (ocfd_set_tuning): launch-shape choices that change no result beyond round-off.
 struct Tuning {
-    int xy_fused;    // 1 (default): x and y sweeps in one kernel; 0: one marching launch per direction (A/B reference)
     int zchunk_f;    // planes per CTA of viscous pass 1 (0 automatic)
     int zchunk_d;    // ... of viscous pass 2
     int zchunk_s;    // ... of the shock sensor
@@ -115,7 +108,6 @@ struct ocfd_ctx {
     unsigned char *flags;  // [3][np] bytes (debug only)
     InvMaps inv;
     MarchMaps march;
-    XYMaps xy;
     CUtensorMap sens_map;   // U with a 1-point x-y halo (stand-alone shock sensor)
     const double *sens_U;
     ViscMaps visc;
@@ -216,7 +208,6 @@ ocfd_status launch_fill_ghosts(ocfd_ctx *c, double *U);
 ocfd_status launch_sensor(ocfd_ctx *c, const double *U);
 ocfd_status launch_flags(ocfd_ctx *c, unsigned char *flags);
 ocfd_status launch_inviscid(ocfd_ctx *c, const double *U, double *dU);
-ocfd_status launch_inviscid_xy(ocfd_ctx *c, const double *U, double *dU);
 ocfd_status launch_inviscid_march(ocfd_ctx *c, const double *U, double *dU, int dir);
 ocfd_status launch_viscous_flux(ocfd_ctx *c, const double *U, bool sensor);
 // RK3 buffers of one stage (eq. 45): out <- a_s Un + b_s (Uin + dt dU); ocfd_rk3_step rotates them so that no stage

@@ -67,6 +67,9 @@ __global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, GasDesc gs, const __
         tma::mbar_wait(&bars[q], 0);
         pressure_plane(gs, ring + q * S_STAGE, tid);
     }
+    // pressure_plane writes a TMA destination in place (generic proxy); the box load that later refills the stage goes
+    // through the async proxy: every thread orders its writes before the barrier that lets tid 0 issue that load
+    tma::fence_proxy_async();
     __syncthreads();
     const int ctr = (ty + 1) * SBX + tx + 2;
     for (int k = k0; k < k1; ++k) {
@@ -97,6 +100,7 @@ __global__ void __launch_bounds__(SNT) k_sensor(GridDesc g, GasDesc gs, const __
             tma::mbar_wait(&bars[sc], ((k + 2 - k0) / S_NST) & 1);
             pressure_plane(gs, ring + sc * S_STAGE, tid);
         }
+        tma::fence_proxy_async();
         __syncthreads();
         if (tid == 0 && k + S_NST <= last) issue(k + S_NST);
     }

@@ -215,6 +215,9 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
         tma::mbar_wait(&bars[q], 0);
         convert_plane<ORDER>(gs, ring + q * VF_STAGE, slots);
     }
+    // convert_plane writes a TMA destination in place (generic proxy); a later box load overwrites the same bytes through
+    // the async proxy, so every thread orders its writes before the barrier that lets tid 0 issue that load
+    tma::fence_proxy_async();
     __syncthreads();
     // whole-tile tests: away from aperiodic faces every point takes the central stencil and no row test is needed
     const bool xin = g.periodic[0] || (i0 >= H && i0 + TX <= g.nx - H);
@@ -335,6 +338,7 @@ __global__ void __launch_bounds__(VNT, ORDER == 8 ? 1 : 2)
             tma::mbar_wait(&bars[sc], ((k + H + 1 - k0) / VF_NST) & 1);
             convert_plane<ORDER>(gs, ring + sc * VF_STAGE, slots);
         }
+        tma::fence_proxy_async();   // generic writes of convert_plane before the async-proxy refill of a stage
         __syncthreads();
         if (tid == 0 && k + VF_NST <= last) issue(k + VF_NST);
     }
