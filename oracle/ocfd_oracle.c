@@ -35,6 +35,7 @@
  *   ora_weno5_masked        (paper boundary scheme, bc_closure) candidate exactness, renormalised weights, no
  *                           out-of-domain reads; the all-shielded value (DESIGN R-21) is PARITY UNPINNED
  *   ora_max_wavespeed       uniform-flow closed form; brute force
+ *   ora_check_state         hand-made fields with known numbers of bad points of each kind (tests/test_oracle_bc.py)
  *   ora_fill_ghosts         BC invariants
  * Unpinned (no data in the container): agreement with the authors' own program output.
  */
@@ -852,6 +853,29 @@ double ora_max_wavespeed(const ora_params *P, const double *U) {
                 if (s > best) best = s;
             }
     return best;
+}
+
+/* ------------------------------------------------------- state guard */
+/* The paper has no divergence handling: the scheme "can be guaranteed not to diverge, provided the time step is
+ * appropriate".  The guard a caller can afford every few steps is a count over interior points:
+ *   counts[0]  points with a NaN or an infinity in any of the five conserved variables,
+ *   counts[1]  points with rho <= 0,
+ *   counts[2]  points with p <= 0, p by eq. 8 (DESIGN R-1) as in prim_of; looked at only where the five values are
+ *              finite and rho > 0 (elsewhere p has no meaning).
+ * A NaN compares false, so a point with NaN rho is in counts[0] only. */
+void ora_check_state(const ora_params *P, const double *U, long long counts[3]) {
+    long np = NP(P);
+    counts[0] = counts[1] = counts[2] = 0;
+    for (int k = 0; k < P->nz; ++k)
+        for (int j = 0; j < P->ny; ++j)
+            for (int i = 0; i < P->nx; ++i) {
+                long id = IDX(P, i, j, k);
+                int finite = 1;
+                for (int m = 0; m < 5; ++m) finite = finite && isfinite(U[m * np + id]);
+                if (!finite) counts[0]++;
+                if (U[id] <= 0.0) counts[1]++;
+                if (finite && U[id] > 0.0 && prim_at(P, U, id).p <= 0.0) counts[2]++;
+            }
 }
 
 /* inviscid term of a single direction only (dU zeroed first), for direction-wise parity tests */

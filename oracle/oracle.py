@@ -232,6 +232,13 @@ class Oracle:
         self._chk(U)
         return self.L.ora_max_wavespeed(C.byref(self.P), _ptr(U))
 
+    def check_state(self, U):
+        """(points with a non-finite conserved variable, points with rho <= 0, points with p <= 0) over the interior."""
+        self._chk(U)
+        counts = (C.c_longlong * 3)()
+        self.L.ora_check_state(C.byref(self.P), _ptr(U), counts)
+        return tuple(int(v) for v in counts)
+
     def sensor(self, U):
         self._chk(U)
         th = np.full(self.shape[1:], np.nan)

@@ -118,3 +118,39 @@ def test_max_wavespeed_closed_form_and_brute_force():
     U2 = U.copy()
     U2[:, :NG] *= 3.0
     assert o.max_wavespeed(np.ascontiguousarray(U2)) == o.max_wavespeed(U)
+
+
+def test_check_state_counts_hand_made_bad_points():
+    """ora_check_state (the paper's only statement on divergence is PAPER.md:L305): known numbers of
+    points of each kind planted by hand in a clean field; ghosts, edges and corners do not take part."""
+    case = W.smooth_periodic(9, 8, 7, grid="wavy")
+    o = Oracle(case)
+    assert o.check_state(case.U0) == (0, 0, 0)
+    U = case.U0.copy()
+    g = case.gamma
+    pts = lambda *ijk: tuple(NG + q for q in reversed(ijk))          # (i, j, k) -> padded [k][j][i]
+    U[(4,) + pts(0, 0, 0)] = np.nan                                    # E NaN: non-finite only
+    U[(1,) + pts(8, 7, 6)] = np.inf                                    # rho u inf: non-finite only (last interior point)
+    U[(0,) + pts(3, 2, 1)] = np.nan                                    # rho NaN: non-finite, NOT rho <= 0 (NaN compares false)
+    U[(0,) + pts(4, 4, 4)] = -0.5                                      # rho < 0: counted once, p not looked at
+    U[(0,) + pts(5, 4, 4)] = 0.0                                       # rho == 0 counts as bad
+    U[(0,) + pts(6, 1, 2)] = -np.inf                                   # -inf rho: non-finite AND rho <= 0
+    for (i, j, k), frac in (((1, 1, 1), 0.5), ((2, 6, 3), 1.0), ((7, 0, 5), 0.999999)):
+        idx = pts(i, j, k)                                             # E below / at / just under the kinetic energy
+        ke = 0.5 * (U[(1,) + idx] ** 2 + U[(2,) + idx] ** 2 + U[(3,) + idx] ** 2) / U[(0,) + idx]
+        U[(4,) + idx] = frac * ke
+    # p = (g-1)(E - ke): 0.5 ke and 0.999999 ke give p < 0; E = ke gives p == 0 up to the rounding of ke, planted as exactly
+    # zero velocity instead so that p == 0 is exact
+    idx = pts(2, 6, 3)
+    U[(1,) + idx] = U[(2,) + idx] = U[(3,) + idx] = 0.0
+    U[(4,) + idx] = 0.0
+    # bad values in ghosts must not count
+    U[0, 0, :, :] = -1.0
+    U[4, :, :, -1] = np.nan
+    assert o.check_state(np.ascontiguousarray(U)) == (4, 3, 3)
+    # a healthy pressure just above zero is not counted
+    V = case.U0.copy()
+    idx = pts(3, 3, 3)
+    ke = 0.5 * (V[(1,) + idx] ** 2 + V[(2,) + idx] ** 2 + V[(3,) + idx] ** 2) / V[(0,) + idx]
+    V[(4,) + idx] = ke + 1e-9 / (g - 1.0)
+    assert o.check_state(V) == (0, 0, 0)
