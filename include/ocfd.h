@@ -135,6 +135,17 @@ ocfd_status ocfd_rk3_steps_host(ocfd_ctx *ctx, double *U_host, double *U_dev, do
  * the caller sets dt = CFL / Lambda.  Writes one double to host_out and synchronises the stream. */
 ocfd_status ocfd_max_wavespeed(ocfd_ctx *ctx, const double *U, double *host_out);
 
+/* State guard.  The paper handles no divergence: the scheme "can be guaranteed not to diverge,
+ * provided the time step is appropriate"; ocfd_max_wavespeed turns a NaN state into a NaN Lambda, but a
+ * negative density or pressure only shows up as a NaN one stage later, without a place or a count.  This call counts,
+ * over the interior points of U (device pointer; ghosts are not looked at):
+ *   host_counts[0]  points with a NaN or an infinity in any of the five conserved variables,
+ *   host_counts[1]  points with rho <= 0 (a NaN rho compares false and is in [0] only; -inf is in both),
+ *   host_counts[2]  points with p = (gamma-1)(E - rho (u^2+v^2+w^2)/2) <= 0, evaluated only where all five values are
+ *                   finite and rho > 0.
+ * One kernel (40 B/point read once), one 24-byte device-to-host copy; returns after the stream has drained. */
+ocfd_status ocfd_check_state(ocfd_ctx *ctx, const double *U, long long host_counts[3]);
+
 /* Row a9 for callers that cannot allocate device memory.  Everything else in this header needs a context, and a
  * context needs a workspace of several fields from the caller; code that must not call cudaMalloc -- a callback inside
  * an application whose own pool already owns all of HBM, a monitoring hook that may not disturb the allocator, a job
@@ -181,7 +192,7 @@ size_t ocfd_sizeof_params(void);
  * synchronises the stream, adds up the elapsed milliseconds and launch counts per class since the last read
  * into ms[OCFD_NKERNELS] / launches[OCFD_NKERNELS] (host arrays) and clears the record.  Class names:
  * ocfd_kernel_name(id), id = 0 .. OCFD_NKERNELS-1. */
-#define OCFD_NKERNELS 9
+#define OCFD_NKERNELS 10
 ocfd_status ocfd_timing(ocfd_ctx *ctx, int enable);
 ocfd_status ocfd_timing_read(ocfd_ctx *ctx, double *ms, long long *launches);
 const char *ocfd_kernel_name(int id);

@@ -19,8 +19,8 @@ OCFD_OK = 0
 EXPORTS = ["ocfd_workspace_bytes", "ocfd_init", "ocfd_destroy", "ocfd_fill_ghosts", "ocfd_rhs", "ocfd_rk3_step",
            "ocfd_rk3_steps_host", "ocfd_max_wavespeed", "ocfd_debug_sensor", "ocfd_timing", "ocfd_timing_read",
            "ocfd_kernel_name", "ocfd_sizeof_params", "ocfd_launch_count", "ocfd_strerror", "ocfd_set_tuning",
-           "ocfd_max_wavespeed_static"]
-NKERNELS = 9
+           "ocfd_max_wavespeed_static", "ocfd_check_state"]
+NKERNELS = 10
 
 
 class OcfdParams(C.Structure):
@@ -81,6 +81,8 @@ def load():
     L.ocfd_max_wavespeed.argtypes = [vp, vp, C.POINTER(C.c_double)]
     L.ocfd_max_wavespeed_static.restype = C.c_int
     L.ocfd_max_wavespeed_static.argtypes = [pp, vp, C.POINTER(C.c_double)]
+    L.ocfd_check_state.restype = C.c_int
+    L.ocfd_check_state.argtypes = [vp, vp, C.POINTER(C.c_longlong)]
     L.ocfd_debug_sensor.restype = C.c_int
     L.ocfd_debug_sensor.argtypes = [vp, vp, vp, vp]
     L.ocfd_launch_count.restype = C.c_longlong
@@ -240,6 +242,12 @@ class Solver:
         out = C.c_double(0.0)
         _check(self.L.ocfd_max_wavespeed(self.ctx, self._ptr(U), C.byref(out)))
         return out.value
+
+    def check_state(self, U):
+        """(points with a non-finite conserved variable, points with rho <= 0, points with p <= 0) over the interior."""
+        counts = (C.c_longlong * 3)()
+        _check(self.L.ocfd_check_state(self.ctx, self._ptr(U), counts))
+        return tuple(int(v) for v in counts)
 
     def debug_sensor(self, U):
         theta = self.torch.full(self.case_shape[1:], float("nan"), dtype=self.torch.float64, device=self.device)

@@ -239,6 +239,12 @@ ocfd_status ocfd_max_wavespeed(ocfd_ctx *c, const double *U, double *host_out) {
     return launch_wavespeed(c, U, host_out);
 }
 
+ocfd_status ocfd_check_state(ocfd_ctx *c, const double *U, long long *host_counts) {
+    if (!live(c)) return OCFD_ESTATE;
+    if (!U || !host_counts) return OCFD_EINVAL;
+    return launch_check_state(c, U, host_counts);
+}
+
 ocfd_status ocfd_debug_sensor(ocfd_ctx *c, const double *U, double *theta, unsigned char *flag_xyz) {
     if (!live(c)) return OCFD_ESTATE;
     if (!U) return OCFD_EINVAL;
@@ -279,7 +285,8 @@ ocfd_status ocfd_timing_read(ocfd_ctx *c, double *ms, long long *launches) {
 
 const char *ocfd_kernel_name(int id) {
     static const char *names[OCFD_NKERNELS] = {"ghost_fill", "shock_sensor", "inviscid_x", "inviscid_y",
-                                               "inviscid_z", "viscous_flux", "viscous_div", "rk3_update", "max_wavespeed"};
+                                               "inviscid_z", "viscous_flux", "viscous_div", "rk3_update", "max_wavespeed",
+                                               "check_state"};
     return id >= 0 && id < OCFD_NKERNELS ? names[id] : "?";
 }
 

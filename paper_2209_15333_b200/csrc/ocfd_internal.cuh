@@ -54,7 +54,7 @@ struct GasDesc {
 };
 
 // kernel classes, for ocfd_timing_read / ocfd_kernel_name (K_INV_X + d = the sweep of direction d as its own launch)
-enum { K_GHOST = 0, K_SENSOR, K_INV_X, K_INV_Y, K_INV_Z, K_VISC_FLUX, K_VISC_DIV, K_RK, K_WAVE, K_COUNT };
+enum { K_GHOST = 0, K_SENSOR, K_INV_X, K_INV_Y, K_INV_Z, K_VISC_FLUX, K_VISC_DIV, K_RK, K_WAVE, K_CHECK, K_COUNT };
 static_assert(K_COUNT == OCFD_NKERNELS, "kernel class count");
 
 struct TimedLaunch { cudaEvent_t a, b; int id; };
@@ -217,6 +217,7 @@ ocfd_status launch_viscous_div(ocfd_ctx *c, double *dU, const RkBufs &rk, double
 ocfd_status launch_rk_update(ocfd_ctx *c, const double *Un, const double *Uin, double *out, const double *dU, double dt,
                              int stage);
 ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out);
+ocfd_status launch_check_state(ocfd_ctx *c, const double *U, long long *host_counts);
 
 // Raise the dynamic shared-memory limit of `kernel` to `bytes` once per context (the attribute lives in the device
 // context of the function, so a process-wide flag would leave a second device without it).

@@ -156,12 +156,16 @@ __global__ void __launch_bounds__(WS_NT) k_wavespeed(GridDesc g, GasDesc gs, con
         };
         if (fixed) fetch(OCFD_NG);
         long long id = pidx(g, ip, jp, k0 + OCFD_NG);
+        // seeded reciprocal and square root (schemes.cuh: within an ulp or two; a NaN, zero or negative argument still
+        // ends as a non-finite s): the library 1/x and sqrt were half of this kernel's instructions; two planes per
+        // trip keep ten loads in flight per thread
+#pragma unroll 2
         for (int k = k0; k < k1; ++k, id += g.sz) {
             if (!fixed) fetch(k + OCFD_NG);
-            const double rho = U[id], ir = 1.0 / rho;
-            const double u = U[g.np + id] * ir, v = U[2 * g.np + id] * ir, w = U[3 * g.np + id] * ir;
-            const double p = gs.gm1 * (U[4 * g.np + id] - 0.5 * rho * (u * u + v * v + w * w));
-            const double c = sqrt(gs.gM2 * p * ir) * gs.invMa;
+            const double rho = __ldcs(U + id), ir = fast_rcp_pos(rho);
+            const double u = __ldcs(U + g.np + id) * ir, v = __ldcs(U + 2 * g.np + id) * ir, w = __ldcs(U + 3 * g.np + id) * ir;
+            const double p = gs.gm1 * (__ldcs(U + 4 * g.np + id) - 0.5 * rho * (u * u + v * v + w * w));
+            const double c = fast_sqrt_pos(gs.gM2 * p * ir) * gs.invMa;
             double s = 0.0;
 #pragma unroll
             for (int d = 0; d < 3; ++d) s += fabs(a[d][0] * u + a[d][1] * v + a[d][2] * w) + c * len[d];
@@ -176,6 +180,37 @@ __global__ void __launch_bounds__(WS_NT) k_wavespeed(GridDesc g, GasDesc gs, con
     bad = __any_sync(0xffffffffu, bad);
     if ((threadIdx.x & 31) == 0)
         atomicMax(out, bad ? 0x7ff8000000000000ull : (unsigned long long)__double_as_longlong(best));
+}
+
+// State guard: counts of interior points with a non-finite conserved variable, with rho <= 0, with p <= 0 (p looked at
+// only where the five values are finite and rho > 0).  Same launch shape as the wavespeed march: one (i, j) column per
+// thread, coalesced along x, 40 B/point read once.  Integer counts: warp-reduced, then one atomic per warp and counter.
+__global__ void __launch_bounds__(WS_NT) k_check_state(GridDesc g, GasDesc gs, const double *__restrict__ U,
+                                                       unsigned long long *__restrict__ counts, int zchunk) {
+    const int i = blockIdx.x * WS_NT + threadIdx.x, j = blockIdx.y;
+    const int k0 = blockIdx.z * zchunk, k1 = min(k0 + zchunk, g.nz);
+    unsigned int n_nonfinite = 0, n_rho = 0, n_p = 0;
+    if (i < g.nx) {
+        long long id = pidx(g, i + OCFD_NG, j + OCFD_NG, k0 + OCFD_NG);
+        for (int k = k0; k < k1; ++k, id += g.sz) {
+            const double rho = U[id], m1 = U[g.np + id], m2 = U[2 * g.np + id], m3 = U[3 * g.np + id], E = U[4 * g.np + id];
+            const bool finite = isfinite(rho) && isfinite(m1) && isfinite(m2) && isfinite(m3) && isfinite(E);
+            n_nonfinite += !finite;
+            n_rho += rho <= 0.0;
+            if (finite && rho > 0.0) {
+                const double u = m1 / rho, v = m2 / rho, w = m3 / rho;
+                n_p += gs.gm1 * (E - 0.5 * rho * (u * u + v * v + w * w)) <= 0.0;
+            }
+        }
+    }
+    n_nonfinite = __reduce_add_sync(0xffffffffu, n_nonfinite);
+    n_rho = __reduce_add_sync(0xffffffffu, n_rho);
+    n_p = __reduce_add_sync(0xffffffffu, n_p);
+    if ((threadIdx.x & 31) == 0) {
+        if (n_nonfinite) atomicAdd(counts, (unsigned long long)n_nonfinite);
+        if (n_rho) atomicAdd(counts + 1, (unsigned long long)n_rho);
+        if (n_p) atomicAdd(counts + 2, (unsigned long long)n_p);
+    }
 }
 
 }  // namespace
@@ -230,6 +265,25 @@ ocfd_status launch_wavespeed(ocfd_ctx *c, const double *U, double *host_out) {
     }
     OCFD_CHECK_LAUNCH(c);
     if (cudaMemcpyAsync(host_out, out, sizeof(double), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return OCFD_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return OCFD_ECUDA;
+    return OCFD_OK;
+}
+
+ocfd_status launch_check_state(ocfd_ctx *c, const double *U, long long *host_counts) {
+    const GridDesc &g = c->g;
+    unsigned long long *cnt = (unsigned long long *)c->scal + 1;   // word 0 of the scalar area is the wavespeed result
+    if (g.ny > 65535) return OCFD_EINVAL;
+    if (cudaMemsetAsync(cnt, 0, 3 * sizeof(unsigned long long), c->stream) != cudaSuccess) return OCFD_ECUDA;
+    int zc = g.nz;
+    const long long cols = (long long)((g.nx + WS_NT - 1) / WS_NT) * g.ny;
+    while (zc > 32 && cols * ((g.nz + zc - 1) / zc) < 8ll * c->nsm) zc = (zc + 1) / 2;
+    if (zc > 64) zc = 64;
+    const dim3 grd((g.nx + WS_NT - 1) / WS_NT, g.ny, (g.nz + zc - 1) / zc);
+    OCFD_T0(c, K_CHECK);
+    k_check_state<<<grd, WS_NT, 0, c->stream>>>(g, c->gas, U, cnt, zc);
+    OCFD_CHECK_LAUNCH(c);
+    if (cudaMemcpyAsync(host_counts, cnt, 3 * sizeof(long long), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+        return OCFD_ECUDA;
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return OCFD_ECUDA;
     return OCFD_OK;
 }
