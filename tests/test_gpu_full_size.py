@@ -153,3 +153,127 @@ def test_config2_hit128_whole_array_rhs_and_three_steps(B, Oracle):
     err3 = max(np.abs(got[m] - U[m]).max() / np.abs(U[m]).max() for m in range(5))
     print("config 2: three RK3 steps rel Linf", err3)
     assert err3 <= 1e-10
+
+
+# ------------------------------------------------------------------ the timed path itself, at full size
+def window_case(case, U_full, box):
+    """The sub-box [i0,i1) x [j0,j1) x [k0,k1) of `case` as a case of its own, for the CPU side only: state (with the
+    true neighbours in its ghost layers), metric planes and boundary data cut out of the full arrays.  A face of the box
+    that is a face of the domain keeps the domain's condition and data; an axis the box spans completely stays periodic
+    if it was; every other face is a CUT face and gets plain extrapolation, which is wrong there -- the error it makes
+    travels 6 points per stage (the reach of the two-pass viscous operator; the inviscid stencils reach 4), so points
+    18 or more away from every cut face see none of it after one RK3 step.  Returns (case, cut[6])."""
+    import dataclasses
+    i0, i1, j0, j1, k0, k1 = box
+    lo, hi, n = (i0, j0, k0), (i1, j1, k1), (case.nx, case.ny, case.nz)
+    sl = {0: slice(i0, i1 + 2 * NG), 1: slice(j0, j1 + 2 * NG), 2: slice(k0, k1 + 2 * NG)}
+    met = []
+    for m in case.metrics:
+        mk = slice(None) if m.shape[0] == 1 else sl[2]
+        met.append(np.ascontiguousarray(m[mk, sl[1], sl[0]]))
+    bc, cut = list(case.bc), [False] * 6
+    inflow, wall_vn = [None] * 6, [None] * 6
+    for d in range(3):
+        whole = lo[d] == 0 and hi[d] == n[d]
+        for side in range(2):
+            f = 2 * d + side
+            on_domain_face = lo[d] == 0 if side == 0 else hi[d] == n[d]
+            if case.bc[f] == "periodic":
+                if not whole:
+                    bc[f], cut[f] = "outflow", True
+                continue
+            if not on_domain_face:
+                bc[f], cut[f] = "outflow", True
+                continue
+            slow, fast = (2, 1) if d == 0 else (2, 0) if d == 1 else (1, 0)      # tangential axes of the face arrays
+            if case.inflow[f] is not None:
+                inflow[f] = np.ascontiguousarray(case.inflow[f][:, sl[slow], sl[fast]])
+            if case.wall_vn[f] is not None:
+                wall_vn[f] = np.ascontiguousarray(case.wall_vn[f][sl[slow], sl[fast]])
+    sub = dataclasses.replace(case, name=f"{case.name}[{i0}:{i1},{j0}:{j1},{k0}:{k1}]", nx=i1 - i0, ny=j1 - j0, nz=k1 - k0,
+                              metrics=met, bc=bc, inflow=inflow, wall_vn=wall_vn, coords=None,
+                              U0=np.ascontiguousarray(U_full[:, sl[2], sl[1], sl[0]]))
+    assert sub.weno_eps == case.weno_eps
+    return sub, cut
+
+
+def test_config5_full_size_one_rk3_step_whole_windows(B, Oracle):
+    """ONE ocfd_rk3_step of config 5 at 2048 x 300 x 256 -- the call, the launch shapes (automatic march segments,
+    z chunks of the viscous passes, CTA numbering, rotating state buffers, fused RK3 update) and the grid bench.py
+    times -- compared with the CPU reference on WHOLE windows, every point of them that no cut face can have reached:
+    the four x-y corners over the full periodic span (inflow / wall / outflow faces, the periodic seam in z, the z-chunk
+    seams k = 32, 64, ...), the ragged last tiles in y (300 = 9*32 + 12 = 37*8 + 4), the seam i = 1024 between the two
+    segments the automatic rule cuts the x march into, the seam i = 512 between two column groups of the viscous CTA
+    numbering, the steepest pressure front of the initial field, and two seeded interior boxes cut in all directions.
+    Interfaces whose sensor value comes within 1e-9 of a threshold at any stage may legitimately decide differently;
+    they are counted and their domain of influence is left out, as in the stepping tests."""
+    import torch
+    from tests.parity_utils import near_threshold, dilate
+    case = W.ramp()
+    assert (case.nx, case.ny, case.nz) == (2048, 300, 256) and case.scheme == "hybrid"
+    nx, ny, nz = case.nx, case.ny, case.nz
+    o_full = Oracle(case)
+    U_full = o_full.fill_ghosts(case.U0.copy())
+    dt = case.cfl / o_full.max_wavespeed(U_full)
+    s = B.Solver(case)
+    Ud = s.to_device(U_full)
+    s.rk3_step(Ud, dt)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(Ud[:, NG:-NG, NG:-NG, NG:-NG]).all())
+    # where the initial pressure is steepest along x (plane k = 10, away from the faces): the flagged region
+    Up = U_full[:, NG + 10, NG:-NG, NG:-NG]
+    p = (case.gamma - 1.0) * (Up[4] - 0.5 * (Up[1] ** 2 + Up[2] ** 2 + Up[3] ** 2) / Up[0])
+    gp = np.abs(p[40:-40, 42:-38] - p[40:-40, 40:-40]) / p[40:-40, 41:-39]
+    jf, i_f = np.unravel_index(int(np.argmax(gp)), gp.shape)
+    jf, i_f = int(jf) + 40, int(i_f) + 41
+    rng = np.random.default_rng(77)
+    boxes = {
+        "corner x- y-": (0, 72, 0, 72, 0, nz), "corner x+ y-": (nx - 72, nx, 0, 72, 0, nz),
+        "corner x- y+ (ragged y tiles)": (0, 72, ny - 72, ny, 0, nz), "corner x+ y+ (ragged y tiles)": (nx - 72, nx, ny - 72, ny, 0, nz),
+        "x march seam i=1024": (1024 - 36, 1024 + 36, 100, 172, 0, nz),
+        "column-group seam i=512, top": (512 - 36, 512 + 36, ny - 72, ny, 0, nz),
+        "steepest pressure front": (max(0, min(nx - 96, i_f - 48)), max(0, min(nx - 96, i_f - 48)) + 96,
+                                    max(0, min(ny - 80, jf - 40)), max(0, min(ny - 80, jf - 40)) + 80, 0, nz),
+    }
+    for q in range(2):
+        a, b, c = int(rng.integers(100, nx - 200)), int(rng.integers(20, ny - 120)), int(rng.integers(8, nz - 140))
+        boxes[f"interior box {q}"] = (a, a + 100, b, b + 100, c, c + 130)
+    M = 18
+    worst, checked, near_total = 0.0, 0, 0
+    for tag, box in boxes.items():
+        sub, cut = window_case(case, U_full, box)
+        o = Oracle(sub)
+        U = sub.U0.copy()
+        Un = U.copy()
+        excl = np.zeros((sub.nz, sub.ny, sub.nx), dtype=bool)
+        per = [sub.bc[2 * d] == "periodic" for d in range(3)]
+        for st in range(3):                                   # the calls ora_rk3_step makes, with a look at theta per stage
+            o.fill_ghosts(U)
+            m = near_threshold(o.sensor(U), sub.theta1, sub.theta2, 1e-9)
+            if m.any():
+                near_total += int(m.sum())
+                excl |= dilate(m, M, per)
+            o.rk3_update(Un, U, o.rhs(U), dt, st)
+        o.fill_ghosts(U)                                      # the step ends with a fill: it resets the wall / inflow nodes
+        keep = ~excl
+        lo = [M if cut[2 * d] else 0 for d in range(3)]
+        hi = [M if cut[2 * d + 1] else 0 for d in range(3)]
+        inner = (slice(lo[2], sub.nz - hi[2]), slice(lo[1], sub.ny - hi[1]), slice(lo[0], sub.nx - hi[0]))
+        i0, i1, j0, j1, k0, k1 = box
+        got = Ud[:, NG + k0:NG + k1, NG + j0:NG + j1, NG + i0:NG + i1].cpu().numpy()
+        ref = U[:, NG:-NG, NG:-NG, NG:-NG]
+        umax = np.abs(ref).max()
+        err = 0.0
+        for mcomp in range(5):
+            d = np.abs(got[mcomp] - ref[mcomp])[inner][keep[inner]]
+            err = max(err, d.max() / max(np.abs(ref[mcomp]).max(), 1e-3 * umax))
+        npts = int(keep[inner].sum())
+        checked += npts
+        worst = max(worst, err)
+        print(f"config 5 full size, one RK3 step, window {tag} {box}: {npts} points compared, rel Linf {err:.3e}, "
+              f"cut faces {cut}")
+        assert npts > 0.15 * sub.nx * sub.ny * sub.nz, tag
+        assert err <= 1e-11, (tag, err)
+    s.close()
+    print(f"config 5 full size: {checked} points in {len(boxes)} windows, worst rel Linf {worst:.3e}, "
+          f"{near_total} points next to an interface within 1e-9 of a threshold (their domain of influence left out)")
