@@ -77,7 +77,13 @@ typedef struct {
     ocfd_scheme scheme;
     double theta1, theta2;   /* hybrid thresholds (0.02, 0.1), theta1 <= theta2; theta2 = +inf gives two
                                 levels */
-    double weno_eps;         /* epsilon of the WENO weights, applied to the J^-1-scaled split flux (DESIGN R-10) */
+    /* epsilon of the WENO weights, applied to the J^-1-scaled split flux (DESIGN R-10).  Range: the kernels form the
+     * WENO7 weights with ONE division, as sum_k P_k C_k q_k / sum_k C_k P_k with P_k a product of three (eps + IS_m)^2,
+     * i.e. of size (eps + IS)^6, and divide by seeded reciprocals that flush subnormal inputs to zero.  That stays in
+     * the normal fp64 range for 1e-50 <= eps + IS <= 1e50, i.e. weno_eps >= 1e-50 (smaller values are OCFD_EINVAL) and
+     * J^-1-scaled split fluxes below about 1e25 in magnitude: any grid and unit system whose cell-face areas lie
+     * between 1e-22 and 1e22 with O(1) non-dimensional flow variables. */
+    double weno_eps;
     double sw_eps;           /* 0: eigenvalue split exactly as eq. 29; > 0: (lambda +- sqrt(lambda^2+eps^2))/2 */
     ocfd_bc bc[6];           /* x-, x+, y-, y+, z-, z+; PERIODIC must be set on both faces of an axis */
     double T_wall[6];        /* non-dimensional wall temperature of WALL faces */
@@ -98,7 +104,8 @@ typedef struct {
      * the domain is computed by WENO5 with the candidate sub-stencils that contain an outside point shielded
      * (weight 0, the others renormalised); no value outside the domain is read by the sweeps.  If all three
      * candidates are shielded (the boundary interface itself, for the wave that enters) the boundary node's split
-     * flux is taken (DESIGN R-21). */
+     * flux is taken (DESIGN R-21).  The paper does not say what happens there: that value is a choice of this build,
+     * matched by the test reference but pinned by nothing in the paper. */
     int bc_closure;
     /* 1: flux reconstruction in characteristic variables (section 2.2.2): at every interface the
      * split fluxes of the stencil are projected with the left eigenvectors S (eq. 35) of the averaged state (eq. 32),

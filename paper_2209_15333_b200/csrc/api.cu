@@ -18,7 +18,7 @@ bool valid_params(const ocfd_params *p) {
     if (p->nx > OCFD_MAX_EXTENT || p->ny > OCFD_MAX_EXTENT || p->nz > OCFD_MAX_EXTENT) return false;  // grid dimensions of the launches
     if (p->nx % 2) return false;  // TMA: row pitch (nx+8)*8 bytes must be a multiple of 16
     if ((long long)(p->nx + 8) * (p->ny + 8) * (p->nz + 8) > (1ll << 40)) return false;
-    if (!(p->gamma > 1.0) || !(p->Ma > 0.0) || !(p->weno_eps > 0.0) || !(p->sw_eps >= 0.0)) return false;
+    if (!(p->gamma > 1.0) || !(p->Ma > 0.0) || !(p->weno_eps >= 1e-50) || !(p->sw_eps >= 0.0)) return false;  // (eps+IS)^6 must stay normal
     if (!p->inviscid && (!(p->Re > 0.0) || !(p->Pr > 0.0) || !(p->T_ref > 0.0) || !(p->T_suth >= 0.0))) return false;
     if (p->scheme < OCFD_UD7 || p->scheme > OCFD_HYBRID) return false;
     if (p->visc_order != 0 && p->visc_order != 6 && p->visc_order != 8) return false;

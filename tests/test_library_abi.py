@@ -43,7 +43,8 @@ def test_params_struct_mirror_and_validation(B):
     assert L.ocfd_workspace_bytes(C.byref(B.params_from_case(case))) < nbytes   # no viscous-flux fields
     # invalid parameters are rejected without touching anything
     for mutate in (lambda p: setattr(p, "ng", 3), lambda p: setattr(p, "nx", 4), lambda p: setattr(p, "gamma", 1.0),
-                   lambda p: setattr(p, "weno_eps", 0.0), lambda p: setattr(p, "scheme", 7),
+                   lambda p: setattr(p, "weno_eps", 0.0), lambda p: setattr(p, "weno_eps", 1e-60),
+                   lambda p: setattr(p, "scheme", 7),
                    lambda p: p.bc.__setitem__(0, B.BCS["outflow"]),          # periodic not paired
                    lambda p: setattr(p, "grid_kind", B.GRID_KINDS["curvilinear"])):   # metrics missing
         Q = B.params_from_case(W.tgv(16))
