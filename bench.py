@@ -367,6 +367,41 @@ def run_ours(args):
     e2e_value = whole_job_value(t_e2e, case.npoints, n_e2e, world, s.device)
     nbytes = int(Uh.numel() * 8)
 
+    # ---- optional: the same fixed-dt steps replayed from a CUDA graph (one graph launch per step instead of 27 kernel
+    # launches), in a second context on a stream of its own (the legacy default stream cannot be captured)
+    graph = None
+    if args.graph:
+        gstream = torch.cuda.Stream()
+        with torch.cuda.stream(gstream):
+            sg = B.Solver(case, device=f"cuda:{local}", stream=gstream)
+            V = U.clone()
+            for _ in range(3):
+                sg.rk3_step(V, dt)
+            gstream.synchronize()
+            cg = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(cg, stream=gstream):
+                sg.rk3_step(V, dt)
+            for _ in range(3):
+                cg.replay()
+            g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            g0.record(gstream)
+            for _ in range(args.steps):
+                cg.replay()
+            g1.record(gstream)
+            gstream.synchronize()
+            ms_graph = g0.elapsed_time(g1)
+            p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            p0.record(gstream)
+            for _ in range(args.steps):
+                sg.rk3_step(V, dt)
+            p1.record(gstream)
+            gstream.synchronize()
+            ms_plain = p0.elapsed_time(p1)
+            sg.close()
+        graph = {"ms_per_step_graph_replay": ms_graph / args.steps, "ms_per_step_plain_launches": ms_plain / args.steps,
+                 "value_graph_replay": case.npoints * args.steps / (ms_graph * 1e-3), "unit": UNIT,
+                 "note": "fixed dt, rows a1-a8, one CUDA-graph launch per step; this rank only"}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -451,6 +486,7 @@ def run_ours(args):
         "roofline": roof,
         "cpu_baseline": cpu,
         "sensor_parity": sensor_parity,
+        "graph": graph,
         "kernels": kern,
     }
     print(json.dumps(line))
@@ -466,6 +502,8 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--graph", action="store_true",
+                    help="also time the fixed-dt steps replayed from a CUDA graph (extra key `graph`; for launch-bound grids)")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="launch-shape knob passed to ocfd_set_tuning (A/B measurements)")
     args = ap.parse_args()

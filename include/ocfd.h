@@ -131,7 +131,10 @@ ocfd_status ocfd_fill_ghosts(ocfd_ctx *ctx, double *U);
 ocfd_status ocfd_rhs(ocfd_ctx *ctx, const double *U, double *dU);
 
 /* Rows a1-a8.  One TVD-RK3 step (eq. 45): 3 x (fill ghosts, RHS, stage update), then a
- * final ghost fill, in place on U. */
+ * final ghost fill, in place on U.  The call only enqueues kernels on the context's stream (27 launches with viscous
+ * terms): after one plain call with the same U pointer (one-time host-side set-up: tensor maps, shared-memory opt-in) it
+ * can be captured into a CUDA graph on a non-default stream and replayed, which is what launch-bound small grids need
+ * (tests/test_gpu_parity.py replays it bit for bit; `bench.py --graph` times it). */
 ocfd_status ocfd_rk3_step(ocfd_ctx *ctx, double *U, double dt);
 
 /* The same nsteps steps end to end from HOST memory: copy U_host (5 padded fields, pinned or pageable) into the

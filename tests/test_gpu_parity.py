@@ -543,6 +543,37 @@ def test_launch_shape_knobs_change_no_bit(B, which):
         assert bool((Ua == Ub).all()), knobs
 
 
+@pytest.mark.parametrize("which", ["tgv", "ramp"])
+def test_rk3_step_replayed_from_a_cuda_graph_gives_the_same_bits(B, which):
+    """ocfd_rk3_step only enqueues kernels on the context's stream, so a caller can capture it into a CUDA graph (after
+    one plain call, which does the one-time host-side set-up) and replay the 27 launches of a step as one graph launch:
+    what small, launch-bound grids need.  Five replays must equal five plain steps bit for bit."""
+    import torch
+    case = W.tgv(24) if which == "tgv" else W.ramp(nx=64, ny=40, nz=16, nmodes=8)
+    stream = torch.cuda.Stream()                     # not the legacy default stream: that one cannot be captured
+    with torch.cuda.stream(stream):
+        s = B.Solver(case, stream=stream)
+        U = s.to_device(case.U0.copy())
+        s.fill_ghosts(U)
+        dt = 0.5 * case.cfl / s.max_wavespeed(U)
+        plain = U.clone()
+        for _ in range(6):
+            s.rk3_step(plain, dt)                    # the first of them is the warm-up call as well
+        V = U.clone()
+        s.rk3_step(V, dt)                            # same buffer as the one captured below
+        stream.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=stream):
+            s.rk3_step(V, dt)
+        # capture enqueues nothing: V still holds the state after one step
+        for _ in range(5):
+            g.replay()
+        stream.synchronize()
+        assert bool((V == plain).all())
+        assert bool(torch.isfinite(V[:, NG:-NG, NG:-NG, NG:-NG]).all())
+        s.close()
+
+
 def test_set_tuning_refuses_what_the_launchers_would_ignore(B):
     """include/ocfd.h: a zchunk value is 0 (automatic) or at least 8; unknown keys and negative values are errors."""
     s = B.Solver(W.smooth_periodic(8, 8, 8))
