@@ -23,6 +23,7 @@
 #include <mutex>
 
 #include "ocfd_internal.cuh"
+#include "schemes.cuh"
 
 namespace {
 
@@ -58,12 +59,13 @@ __global__ void __launch_bounds__(WSS_NT) k_wavespeed_partials(GridDesc g, GasDe
         };
         if (fixed) fetch(OCFD_NG);
         long long id = pidx(g, ip, jp, k0 + OCFD_NG);
+#pragma unroll 2
         for (int k = k0; k < k1; ++k, id += g.sz) {
             if (!fixed) fetch(k + OCFD_NG);
-            const double rho = U[id], ir = 1.0 / rho;
-            const double u = U[g.np + id] * ir, v = U[2 * g.np + id] * ir, w = U[3 * g.np + id] * ir;
-            const double p = gs.gm1 * (U[4 * g.np + id] - 0.5 * rho * (u * u + v * v + w * w));
-            const double c = sqrt(gs.gM2 * p * ir) * gs.invMa;
+            const double rho = __ldcs(U + id), ir = fast_rcp_pos(rho);
+            const double u = __ldcs(U + g.np + id) * ir, v = __ldcs(U + 2 * g.np + id) * ir, w = __ldcs(U + 3 * g.np + id) * ir;
+            const double p = gs.gm1 * (__ldcs(U + 4 * g.np + id) - 0.5 * rho * (u * u + v * v + w * w));
+            const double c = fast_sqrt_pos(gs.gM2 * p * ir) * gs.invMa;
             double s = 0.0;
 #pragma unroll
             for (int d = 0; d < 3; ++d) s += fabs(a[d][0] * u + a[d][1] * v + a[d][2] * w) + c * len[d];
